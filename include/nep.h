@@ -1,0 +1,165 @@
+/*
+ * nep.h -- C ABI of libnep_b200: one training step of a neuroevolution potential (NEP) on one B200.
+ *
+ * The calls follow the paper's statement of the problem (arxiv/paper_2606_19557, "TorchNEP").
+ * P:NNN = line NNN of the paper text; "DESIGN C<k>" = DESIGN.md section 3, step k.
+ *
+ *   model inputs   : species, cutoffs, n_max, basis sizes, l_max, neurons        Table I
+ *   data           : positions, boxes, types, energy / force / virial labels      Eqs. 5-7
+ *   geometry cache : neighbour lists, displacement vectors, basis aggregates,
+ *                    built once and kept on the GPU
+ *   step           : descriptors (Eqs. 15-20) -> network (Eq. 3) -> E, F, W ->
+ *                    loss (Eqs. 4-7) -> analytic gradient (Eq. 8) -> Adam  Eqs. 9-13
+ *
+ * Conventions
+ *   - Opaque context; one context = one CUDA device + one stream; not thread-safe per context.
+ *   - Every call returns 0 (NEP_OK) or a negative NEP_E* code; nep_last_error() gives the message
+ *     (NUL-terminated, owned by the context, valid until the next call on it).  No C++ exception
+ *     crosses the ABI.  Nothing is truncated silently: exceeding a capacity is NEP_ECAPACITY.
+ *   - "host" pointers are plain host memory, borrowed for the duration of the call only.
+ *     "device" pointers are CUDA device memory on the context's device.
+ *   - Device memory is obtained through the caller's allocator callbacks (the Python binding
+ *     implements them with torch tensors).  If `alloc` is NULL the library uses cudaMalloc/cudaFree.
+ *   - Step calls (nep_forward / nep_loss_grad / nep_adam_step) enqueue work on the context's stream
+ *     and return without synchronising unless a host output is requested.
+ *   - There is no CPU fallback: without a CUDA device nep_create fails with NEP_ECUDA.
+ *
+ * Layouts (DESIGN C0)
+ *   theta  : for each species t: w0[t] (neurons x D, row-major), b0[t] (neurons), w1[t] (neurons);
+ *            then b1; then cR[t_i][t_j][n][k]; then cA[t_i][t_j][n][k].   n = 0..n_max, k = 0..basis_size.
+ *   q      : radial n -> n; 3-body (l, n) -> n_R + (l-1) n_A + n; 4-body n -> n_R + l3 n_A + n; 5-body next.
+ *   box    : 9 doubles per structure, rows are the cell vectors a, b, c.
+ *   virial : 9 values per structure, row-major xx xy xz yx yy yz zx zy zz; W = -sum d (x) dE/dd (eV).
+ */
+#ifndef NEP_B200_H
+#define NEP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NEP_OK 0
+#define NEP_EINVAL (-1)    /* bad argument */
+#define NEP_ESTATE (-2)    /* call out of order */
+#define NEP_ECUDA (-3)     /* CUDA runtime error (message holds cudaGetErrorString) */
+#define NEP_ENOMEM (-4)    /* allocator returned NULL */
+#define NEP_ECAPACITY (-5) /* an internal capacity would be exceeded */
+
+typedef struct nep_ctx nep_ctx;
+
+/* Device allocator callbacks.  alloc returns a device pointer aligned to >= 256 bytes, or NULL. */
+typedef void* (*nep_alloc_fn)(void* user, size_t nbytes);
+typedef void (*nep_free_fn)(void* user, void* ptr);
+
+/* Library version string, e.g. "nep_b200 0.1 (sm_100a)". */
+const char* nep_version(void);
+
+/* Model definition (Table I).  1 <= n_species <= 16 (the paper's largest set);
+ * 0 < rc_A <= rc_R (DESIGN G22); n_max >= 0; 1 <= basis <= 16; l_max_3b == 4; l_max_4b in {0,2};
+ * l_max_5b in {0,1} (Table I: "l_max 4 2 1"); neurons >= 1.
+ * cuda_stream: a cudaStream_t (NULL = default stream).  alloc/free_/alloc_user: see above.
+ * On success *out owns the context; release with nep_destroy. */
+int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max_R, int n_max_A,
+               int basis_R, int basis_A, int l_max_3b, int l_max_4b, int l_max_5b, int neurons,
+               nep_alloc_fn alloc, nep_free_fn free_, void* alloc_user, void* cuda_stream);
+
+/* Releases every device buffer through free_ and the context itself.  NULL is a no-op. */
+int nep_destroy(nep_ctx* ctx);
+
+/* Message of the last failing call on ctx ("" if none).  ctx == NULL: message of a failed nep_create. */
+const char* nep_last_error(const nep_ctx* ctx);
+
+/* D = (n_max_R+1) + (n_max_A+1) * (l3 + [l4>0] + [l5>0])  and
+ * N_par = T (D+2) H + 1 + T^2 [(n_max_R+1)(basis_R+1) + (n_max_A+1)(basis_A+1)]   (pinned by Table II). */
+int nep_num_descriptors(const nep_ctx* ctx);
+int64_t nep_num_params(const nep_ctx* ctx);
+
+/* Structures and labels (host, copied to the device).  Replaces any previously loaded set.
+ *   n_atoms [S]; pos [sum N][3] Cartesian, Angstrom; box [S][9]; type [sum N] in 0..T-1;
+ *   E [S] eV (total energy, Eq. 5); F [sum N][3] eV/A (Eq. 6); W [S][9] eV (Eq. 7);
+ *   has_virial [S] 0/1 or NULL = all (DESIGN G14).  E, F, W may all be NULL (predict only; labels can be
+ *   attached later with nep_set_labels).
+ * NEP_EINVAL for non-finite input, det(box) <= 0, type out of range, or a position whose fractional
+ * coordinate is outside [0,1) (wrap first; tolerance 1e-9). */
+int nep_load_structures(nep_ctx* ctx, int n_struct, const int* n_atoms, const double* pos, const double* box,
+                        const int* type, const double* E, const double* F, const double* W,
+                        const unsigned char* has_virial);
+
+/* Attach / replace labels of the loaded set (same shapes as above; all three required). */
+int nep_set_labels(nep_ctx* ctx, const double* E, const double* F, const double* W, const unsigned char* has_virial);
+
+/* S0a + S0b: neighbour lists of every loaded structure for both cutoffs -- all periodic
+ * images (j, n) != (i, 0) with |d| < rc, d = (((r_j - r_i) + n_a a) + n_b b) + n_c c in IEEE fp64 without
+ * FMA (DESIGN C1), ascending (j, n_a, n_b, n_c) per atom -- then the per-pair geometry cache and the
+ * per-atom radial basis aggregate.  Selects the full set as the current batch. */
+int nep_build_neighbors(nep_ctx* ctx);
+
+/* Reads the lists back to the host (parity checks need no internals).  which: 0 = radial, 1 = angular.
+ * Two-call pattern: with j == NULL only *n_pairs and offsets (if non-NULL) are written.
+ * offsets [sum N + 1] (int64); j [P] = neighbour index local to the structure; shift [P][3] = (n_a,n_b,n_c). */
+int nep_get_neighbors(nep_ctx* ctx, int which, int64_t* n_pairs, int64_t* offsets, int* j, signed char* shift);
+
+/* Parameters, gradient and optimiser state: host arrays of N_par floats, layout above.
+ * nep_get_grad returns g = grad_theta L of the last nep_loss_grad (Eq. 8). */
+int nep_set_params(nep_ctx* ctx, const float* theta);
+int nep_get_params(nep_ctx* ctx, float* theta);
+int nep_get_grad(nep_ctx* ctx, float* g);
+/* Overwrites the stored gradient (parity runs feed the same g to both optimisers; also allows external gradients). */
+int nep_set_grad(nep_ctx* ctx, const float* g);
+int nep_set_adam_state(nep_ctx* ctx, const float* m, const float* v, const float* vmax, int64_t t);
+int nep_get_adam_state(nep_ctx* ctx, float* m, float* v, float* vmax, int64_t* t);
+
+/* Descriptor scaler of Eq. 2: s = 1 / (max - min) of each component over every atom of the
+ * loaded set at the current parameters; constant afterwards (no gradient flows through it).
+ * compute needs neighbours and parameters; set/get exchange D doubles with the host. */
+int nep_compute_scaler(nep_ctx* ctx);
+int nep_set_scaler(nep_ctx* ctx, const double* s);
+int nep_get_scaler(nep_ctx* ctx, double* s);
+
+/* Mini-batch = a list of structure ids ("batch" of Table I).  ids == NULL: the whole set.
+ * ids are copied to the device; the same id must not appear twice. */
+int nep_set_batch(nep_ctx* ctx, int n, const int* struct_ids);
+
+/* S1-S5: descriptors, network, energies (Eq. 1), forces and virials (P:145 closed forms) of the batch.
+ *   E_out [S_b], F_out [N_b][3], W_out [S_b][9], all float, in batch order (atoms in the order of ids);
+ *   each may be NULL.  outputs_on_host != 0: host pointers (the call synchronises); else device pointers.
+ * Results are kept inside the context for nep_loss_grad. */
+int nep_forward(nep_ctx* ctx, void* E_out, void* F_out, void* W_out, int outputs_on_host);
+
+/* Unscaled descriptors q [N_b][D] (float, host) of the current batch, from the last nep_forward. */
+int nep_get_descriptors(nep_ctx* ctx, float* q);
+
+/* S6-S9: L = lE dE + lF dF + lV dV (Eqs. 4-7, batch normalisers) and g = grad_theta L with respect to every
+ * network weight and descriptor coefficient (Eq. 8; DESIGN C9-C12).  Needs nep_forward on the same batch
+ * and parameters immediately before (NEP_ESTATE otherwise) and labels.  loss4_host: {L, dE, dF, dV} as
+ * doubles on the host (synchronises) or NULL (stays on the device; see nep_get_loss). */
+int nep_loss_grad(nep_ctx* ctx, double lambda_E, double lambda_F, double lambda_V, double* loss4_host);
+int nep_get_loss(nep_ctx* ctx, double* loss4_host);
+
+/* S10: Adam with AMSGrad on theta with the stored gradient.  variant 0 = Eqs. 9-13 literally (running max of
+ * the bias-corrected second moment, epsilon inside the root); variant 1 = torch.optim.Adam(amsgrad=True).
+ * Increments the step count t.  Invalidates the forward results. */
+int nep_adam_step(nep_ctx* ctx, double lr, double beta1, double beta2, double eps, int variant);
+
+/* Blocks until the context's stream is idle. */
+int nep_synchronize(nep_ctx* ctx);
+
+/* Measurement aids.  launch_count: kernels launched by this context since creation.
+ * Profiling: when enabled, every kernel launch of the step calls is bracketed by CUDA events on the
+ * context's stream; nep_profile_read returns, for up to `cap` distinct kernels, name pointers (static
+ * strings), accumulated milliseconds and launch counts, and resets the accumulators.  Returns the number
+ * of kernels through *n. */
+int nep_launch_count(nep_ctx* ctx, int64_t* n);
+int nep_profile_enable(nep_ctx* ctx, int on);
+int nep_profile_read(nep_ctx* ctx, int cap, const char** names, double* ms, int64_t* launches, int* n);
+
+/* Sizes of the loaded set / current batch: {S, N, P_R, P_A, S_b, N_b, P_R_b, P_A_b}. */
+int nep_get_sizes(nep_ctx* ctx, int64_t* sizes8);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEP_B200_H */

@@ -1,0 +1,612 @@
+// nep_api.cu -- C ABI entry points of libnep_b200 (include/nep.h): argument checks, state machine,
+// host<->device marshalling.  All arithmetic of the step lives in the kernels of the other .cu files.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "nep_internal.h"
+
+static thread_local std::string g_create_error;
+
+namespace nep {
+
+int fail(nep_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+
+void* dev_alloc(nep_ctx* c, size_t bytes)
+{
+    if (bytes == 0) bytes = 256;
+    void* p = nullptr;
+    if (c->alloc) p = c->alloc(c->user, bytes);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+    if (!p) { c->err = "device allocation of " + std::to_string(bytes) + " bytes failed"; return nullptr; }
+    c->allocs.push_back(p);
+    return p;
+}
+
+void dev_free(nep_ctx* c, void* p)
+{
+    if (!p) return;
+    auto it = std::find(c->allocs.begin(), c->allocs.end(), p);
+    if (it != c->allocs.end()) c->allocs.erase(it);
+    if (c->alloc) { if (c->free_) c->free_(c->user, p); }
+    else cudaFree(p);
+}
+
+void prof_begin(nep_ctx* c, const char* name)
+{
+    ++c->launches;
+    if (!c->prof.on) return;
+    Profiler::Rec r; r.name = name;
+    auto get = [&]() { cudaEvent_t e; if (!c->prof.pool.empty()) { e = c->prof.pool.back(); c->prof.pool.pop_back(); } else cudaEventCreate(&e); return e; };
+    r.a = get(); r.b = get();
+    cudaEventRecord(r.a, c->stream);
+    c->prof.pending.push_back(r);
+}
+void prof_end(nep_ctx* c)
+{
+    if (!c->prof.on) return;
+    cudaEventRecord(c->prof.pending.back().b, c->stream);
+}
+
+}  // namespace nep
+
+using namespace nep;
+
+#define CHECK_CTX(c) do { if (!(c)) return NEP_EINVAL; } while (0)
+#define ALLOC(c, ptr, type, count)                                              \
+    do {                                                                        \
+        (ptr) = (type*)dev_alloc((c), sizeof(type) * (size_t)(count));          \
+        if (!(ptr)) return NEP_ENOMEM;                                          \
+    } while (0)
+
+template <class T>
+static int upload(nep_ctx* c, T*& dptr, const T* h, size_t count)
+{
+    dptr = (T*)dev_alloc(c, sizeof(T) * std::max<size_t>(count, 1));
+    if (!dptr) return NEP_ENOMEM;
+    if (count) NEP_CUDA(c, cudaMemcpyAsync(dptr, h, sizeof(T) * count, cudaMemcpyHostToDevice, c->stream));
+    return NEP_OK;
+}
+
+extern "C" {
+
+const char* nep_version(void) { return "nep_b200 0.1 (sm_100a, fp32 step, fp64 neighbour predicate)"; }
+
+const char* nep_last_error(const nep_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max_R, int n_max_A, int basis_R, int basis_A,
+               int l_max_3b, int l_max_4b, int l_max_5b, int neurons, nep_alloc_fn alloc, nep_free_fn free_, void* alloc_user,
+               void* cuda_stream)
+{
+    if (!out) return fail(nullptr, NEP_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (n_species < 1 || n_species > MAX_T) return fail(nullptr, NEP_EINVAL, "n_species must be in 1..16");
+    if (!(rc_A > 0.0) || !(rc_A <= rc_R) || !std::isfinite(rc_R)) return fail(nullptr, NEP_EINVAL, "need 0 < rc_A <= rc_R");
+    if (n_max_R < 0 || n_max_A < 0 || n_max_R > 19 || n_max_A > 19) return fail(nullptr, NEP_EINVAL, "n_max must be in 0..19");
+    if (basis_R < 1 || basis_A < 1 || basis_R > 16 || basis_A > 16) return fail(nullptr, NEP_EINVAL, "basis_size must be in 1..16");
+    if (l_max_3b != 4) return fail(nullptr, NEP_EINVAL, "l_max_3b must be 4");
+    if (!(l_max_4b == 0 || l_max_4b == 2)) return fail(nullptr, NEP_EINVAL, "l_max_4b must be 0 or 2");
+    if (!(l_max_5b == 0 || l_max_5b == 1)) return fail(nullptr, NEP_EINVAL, "l_max_5b must be 0 or 1");
+    if (neurons < 1 || neurons > 512) return fail(nullptr, NEP_EINVAL, "neurons must be in 1..512");
+    if ((alloc == nullptr) != (free_ == nullptr)) return fail(nullptr, NEP_EINVAL, "alloc and free_ must both be given or both be NULL");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, NEP_ECUDA, "no CUDA device: libnep_b200 has no CPU fallback");
+    }
+    nep_ctx* c = new (std::nothrow) nep_ctx();
+    if (!c) return fail(nullptr, NEP_ENOMEM, "host allocation failed");
+    c->rcR = rc_R; c->rcA = rc_A; c->n_max_R = n_max_R; c->n_max_A = n_max_A; c->basis_R = basis_R; c->basis_A = basis_A;
+    c->l3 = l_max_3b; c->l4 = l_max_4b; c->l5 = l_max_5b;
+    c->alloc = alloc; c->free_ = free_; c->user = alloc_user; c->stream = (cudaStream_t)cuda_stream;
+    ModelDev& m = c->m;
+    m.T = n_species; m.nR = n_max_R + 1; m.nA = n_max_A + 1; m.KR = basis_R + 1; m.KA = basis_A + 1; m.KRP = (m.KR + 3) & ~3;
+    m.H = neurons; m.has4 = l_max_4b > 0; m.has5 = l_max_5b > 0; m.nang = 4 + m.has4 + m.has5;
+    m.D = m.nR + m.nA * m.nang; m.DP = (m.D + 7) & ~7; m.HP = (m.H + 7) & ~7;
+    m.rcR = (float)rc_R; m.rcA = (float)rc_A; m.rcinvR = (float)(1.0 / rc_R); m.rcinvA = (float)(1.0 / rc_A);
+    m.per_type = (m.D + 2) * m.H; m.o_b1 = m.per_type * m.T; m.o_cR = m.o_b1 + 1; m.o_cA = m.o_cR + m.T * m.T * m.nR * m.KR;
+    m.npar = m.o_cA + m.T * m.T * m.nA * m.KA;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&c->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    size_t np = (size_t)m.npar;
+    c->theta = (float*)dev_alloc(c, 4 * np); c->g = (float*)dev_alloc(c, 4 * np); c->am = (float*)dev_alloc(c, 4 * np);
+    c->av = (float*)dev_alloc(c, 4 * np); c->avmax = (float*)dev_alloc(c, 4 * np); c->scaler = (float*)dev_alloc(c, 4 * (size_t)m.DP);
+    if (!c->theta || !c->g || !c->am || !c->av || !c->avmax || !c->scaler) {
+        g_create_error = c->err; nep_destroy(c); return NEP_ENOMEM;
+    }
+    cudaMemsetAsync(c->g, 0, 4 * np, c->stream); cudaMemsetAsync(c->am, 0, 4 * np, c->stream);
+    cudaMemsetAsync(c->av, 0, 4 * np, c->stream); cudaMemsetAsync(c->avmax, 0, 4 * np, c->stream);
+    cudaMemsetAsync(c->theta, 0, 4 * np, c->stream);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) {
+        g_create_error = std::string("CUDA error in nep_create: ") + cudaGetErrorString(cudaGetLastError());
+        nep_destroy(c); return NEP_ECUDA;
+    }
+    *out = c;
+    return NEP_OK;
+}
+
+int nep_destroy(nep_ctx* c)
+{
+    if (!c) return NEP_OK;
+    cudaStreamSynchronize(c->stream);
+    std::vector<void*> a = c->allocs;
+    for (void* p : a) dev_free(c, p);
+    for (auto& r : c->prof.pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto e : c->prof.pool) cudaEventDestroy(e);
+    delete c;
+    return NEP_OK;
+}
+
+int nep_num_descriptors(const nep_ctx* c) { return c ? c->m.D : NEP_EINVAL; }
+int64_t nep_num_params(const nep_ctx* c) { return c ? c->m.npar : NEP_EINVAL; }
+
+static void free_dataset(nep_ctx* c)
+{
+    DataDev& d = c->d;
+    const void* ptrs[] = { d.pos, d.box, d.type, d.atom_off, d.pbase, d.type_p, d.slice_struct, d.Elab, d.Flab, d.Wlab, d.hasv,
+                           d.offR, d.jR, d.shR, d.offA, d.jA, d.shA, d.cntR, d.recoffR, d.recR, d.cntA, d.recoffA, d.recA, d.B };
+    for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
+    memset(&d, 0, sizeof d);
+    c->have_data = c->have_labels = c->have_nbrs = c->forward_valid = c->grad_valid = false;
+}
+
+static int upload_labels(nep_ctx* c, const double* E, const double* F, const double* W, const unsigned char* hv)
+{
+    DataDev& d = c->d;
+    dev_free(c, (void*)d.Elab); dev_free(c, (void*)d.Flab); dev_free(c, (void*)d.Wlab); dev_free(c, (void*)d.hasv);
+    d.Elab = nullptr; d.Flab = nullptr; d.Wlab = nullptr; d.hasv = nullptr;
+    for (int64_t i = 0; i < c->S; ++i) if (!std::isfinite(E[i])) return fail(c, NEP_EINVAL, "non-finite energy label");
+    for (int64_t i = 0; i < 3 * c->N; ++i) if (!std::isfinite(F[i])) return fail(c, NEP_EINVAL, "non-finite force label");
+    for (int64_t i = 0; i < 9 * (int64_t)c->S; ++i) if (!std::isfinite(W[i])) return fail(c, NEP_EINVAL, "non-finite virial label");
+    std::vector<float> Fp((size_t)3 * c->NP, 0.0f), Wf((size_t)9 * c->S);
+    for (int s = 0; s < c->S; ++s)
+        for (int i = 0; i < c->h_nat[s]; ++i)
+            for (int k = 0; k < 3; ++k) Fp[(size_t)k * c->NP + c->h_pbase[s] + i] = (float)F[3 * (c->h_aoff[s] + i) + k];
+    for (size_t i = 0; i < Wf.size(); ++i) Wf[i] = (float)W[i];
+    c->h_hasv.assign(c->S, 1);
+    if (hv) for (int s = 0; s < c->S; ++s) c->h_hasv[s] = hv[s] ? 1 : 0;
+    double* dE; float *dF, *dW; unsigned char* dh;
+    int rc;
+    if ((rc = upload<double>(c, dE, E, c->S))) return rc;
+    if ((rc = upload<float>(c, dF, Fp.data(), Fp.size()))) return rc;
+    if ((rc = upload<float>(c, dW, Wf.data(), Wf.size()))) return rc;
+    if ((rc = upload<unsigned char>(c, dh, c->h_hasv.data(), c->S))) return rc;
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    d.Elab = dE; d.Flab = dF; d.Wlab = dW; d.hasv = dh;
+    c->have_labels = true;
+    c->grad_valid = false;
+    return NEP_OK;
+}
+
+int nep_load_structures(nep_ctx* c, int S, const int* n_atoms, const double* pos, const double* box, const int* type,
+                        const double* E, const double* F, const double* W, const unsigned char* has_virial)
+{
+    CHECK_CTX(c);
+    if (S < 0 || (S > 0 && (!n_atoms || !pos || !box || !type))) return fail(c, NEP_EINVAL, "NULL input array");
+    bool lab = E || F || W;
+    if (lab && !(E && F && W)) return fail(c, NEP_EINVAL, "E, F and W must be given together");
+    std::vector<int64_t> aoff(S + 1, 0), pbase(S + 1, 0);
+    for (int s = 0; s < S; ++s) {
+        if (n_atoms[s] < 1) return fail(c, NEP_EINVAL, "structure with no atoms");
+        aoff[s + 1] = aoff[s] + n_atoms[s];
+        pbase[s + 1] = pbase[s] + ((n_atoms[s] + WARP - 1) / WARP) * WARP;
+    }
+    int64_t N = aoff[S], NP = pbase[S];
+    if (NP / WARP > (int64_t)INT32_MAX / 4) return fail(c, NEP_ECAPACITY, "too many atoms");
+    for (int s = 0; s < S; ++s) {
+        const double* b = box + 9 * s;
+        for (int k = 0; k < 9; ++k) if (!std::isfinite(b[k])) return fail(c, NEP_EINVAL, "non-finite box");
+        double det = b[0] * (b[4] * b[8] - b[5] * b[7]) - b[1] * (b[3] * b[8] - b[5] * b[6]) + b[2] * (b[3] * b[7] - b[4] * b[6]);
+        if (!(det > 0.0)) return fail(c, NEP_EINVAL, "det(box) <= 0 for structure " + std::to_string(s));
+        // inverse (columns = reciprocal vectors / det): frac = r . inv
+        double inv[9] = { (b[4] * b[8] - b[5] * b[7]) / det, (b[2] * b[7] - b[1] * b[8]) / det, (b[1] * b[5] - b[2] * b[4]) / det,
+                          (b[5] * b[6] - b[3] * b[8]) / det, (b[0] * b[8] - b[2] * b[6]) / det, (b[2] * b[3] - b[0] * b[5]) / det,
+                          (b[3] * b[7] - b[4] * b[6]) / det, (b[1] * b[6] - b[0] * b[7]) / det, (b[0] * b[4] - b[1] * b[3]) / det };
+        for (int64_t i = aoff[s]; i < aoff[s + 1]; ++i) {
+            const double* r = pos + 3 * i;
+            if (!std::isfinite(r[0]) || !std::isfinite(r[1]) || !std::isfinite(r[2])) return fail(c, NEP_EINVAL, "non-finite position");
+            if (type[i] < 0 || type[i] >= c->m.T) return fail(c, NEP_EINVAL, "type out of range at atom " + std::to_string(i));
+            for (int k = 0; k < 3; ++k) {
+                double f = r[0] * inv[k] + r[1] * inv[3 + k] + r[2] * inv[6 + k];
+                if (f < -1e-9 || f >= 1.0 + 1e-9)
+                    return fail(c, NEP_EINVAL, "fractional coordinate outside [0,1) at atom " + std::to_string(i) + " (wrap positions first)");
+            }
+        }
+    }
+    free_dataset(c);
+    c->S = S; c->N = N; c->NP = NP; c->nslices = (int)(NP / WARP);
+    c->h_nat.assign(n_atoms, n_atoms + S); c->h_aoff = aoff; c->h_pbase = pbase; c->h_box.assign(box, box + 9 * (size_t)S);
+    std::vector<int> type_p((size_t)NP, -1), slice_struct((size_t)c->nslices, 0);
+    for (int s = 0; s < S; ++s) {
+        for (int i = 0; i < n_atoms[s]; ++i) type_p[pbase[s] + i] = type[aoff[s] + i];
+        for (int64_t sl = pbase[s] / WARP; sl < pbase[s + 1] / WARP; ++sl) slice_struct[sl] = s;
+    }
+    DataDev& d = c->d;
+    d.S = S; d.N = N; d.NP = NP; d.nslices = c->nslices;
+    int rc;
+    double *dpos, *dbox; int *dtype, *dtp, *dss; int64_t *dao, *dpb;
+    if ((rc = upload<double>(c, dpos, pos, 3 * (size_t)N))) return rc;
+    if ((rc = upload<double>(c, dbox, box, 9 * (size_t)S))) return rc;
+    if ((rc = upload<int>(c, dtype, type, (size_t)N))) return rc;
+    if ((rc = upload<int>(c, dtp, type_p.data(), type_p.size()))) return rc;
+    if ((rc = upload<int>(c, dss, slice_struct.data(), slice_struct.size()))) return rc;
+    if ((rc = upload<int64_t>(c, dao, aoff.data(), aoff.size()))) return rc;
+    if ((rc = upload<int64_t>(c, dpb, pbase.data(), pbase.size()))) return rc;
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    d.pos = dpos; d.box = dbox; d.type = dtype; d.type_p = dtp; d.slice_struct = dss; d.atom_off = dao; d.pbase = dpb;
+    c->have_data = true;
+    if (lab) return upload_labels(c, E, F, W, has_virial);
+    c->h_hasv.assign(S, 1);
+    return NEP_OK;
+}
+
+int nep_set_labels(nep_ctx* c, const double* E, const double* F, const double* W, const unsigned char* has_virial)
+{
+    CHECK_CTX(c);
+    if (!c->have_data) return fail(c, NEP_ESTATE, "nep_set_labels before nep_load_structures");
+    if (!E || !F || !W) return fail(c, NEP_EINVAL, "E, F and W are all required");
+    int rc = upload_labels(c, E, F, W, has_virial);
+    if (rc == NEP_OK && c->have_nbrs) {   // Sv of the current batch depends on the mask
+        int sv = 0;
+        for (int sid : c->h_bsid) sv += c->h_hasv[sid];
+        c->b.Sv = sv;
+    }
+    return rc;
+}
+
+int nep_build_neighbors(nep_ctx* c)
+{
+    CHECK_CTX(c);
+    if (!c->have_data) return fail(c, NEP_ESTATE, "nep_build_neighbors before nep_load_structures");
+    int rc = build_neighbors_dev(c);
+    if (rc) return rc;
+    c->have_nbrs = true;
+    return nep_set_batch(c, 0, nullptr);
+}
+
+int nep_get_neighbors(nep_ctx* c, int which, int64_t* n_pairs, int64_t* offsets, int* j, signed char* shift)
+{
+    CHECK_CTX(c);
+    if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_get_neighbors before nep_build_neighbors");
+    if (which != 0 && which != 1) return fail(c, NEP_EINVAL, "which must be 0 (radial) or 1 (angular)");
+    int64_t P = which ? c->PA : c->PR;
+    if (n_pairs) *n_pairs = P;
+    const DataDev& d = c->d;
+    if (offsets) NEP_CUDA(c, cudaMemcpyAsync(offsets, which ? d.offA : d.offR, 8 * (size_t)(c->N + 1), cudaMemcpyDeviceToHost, c->stream));
+    if (j && P) NEP_CUDA(c, cudaMemcpyAsync(j, which ? d.jA : d.jR, 4 * (size_t)P, cudaMemcpyDeviceToHost, c->stream));
+    if (shift && P) NEP_CUDA(c, cudaMemcpyAsync(shift, which ? d.shA : d.shR, 3 * (size_t)P, cudaMemcpyDeviceToHost, c->stream));
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NEP_OK;
+}
+
+static int h2d(nep_ctx* c, void* dst, const void* src, size_t bytes)
+{
+    NEP_CUDA(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream));
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NEP_OK;
+}
+static int d2h(nep_ctx* c, void* dst, const void* src, size_t bytes)
+{
+    NEP_CUDA(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NEP_OK;
+}
+
+int nep_set_params(nep_ctx* c, const float* theta)
+{
+    CHECK_CTX(c);
+    if (!theta) return fail(c, NEP_EINVAL, "theta is NULL");
+    for (int i = 0; i < c->m.npar; ++i) if (!std::isfinite(theta[i])) return fail(c, NEP_EINVAL, "non-finite parameter");
+    c->have_params = true; c->forward_valid = c->grad_valid = false;
+    return h2d(c, c->theta, theta, 4 * (size_t)c->m.npar);
+}
+int nep_get_params(nep_ctx* c, float* theta)
+{
+    CHECK_CTX(c);
+    if (!theta) return fail(c, NEP_EINVAL, "theta is NULL");
+    return d2h(c, theta, c->theta, 4 * (size_t)c->m.npar);
+}
+int nep_get_grad(nep_ctx* c, float* g)
+{
+    CHECK_CTX(c);
+    if (!g) return fail(c, NEP_EINVAL, "g is NULL");
+    if (!c->grad_valid) return fail(c, NEP_ESTATE, "no gradient: call nep_loss_grad (or nep_set_grad) first");
+    return d2h(c, g, c->g, 4 * (size_t)c->m.npar);
+}
+int nep_set_grad(nep_ctx* c, const float* g)
+{
+    CHECK_CTX(c);
+    if (!g) return fail(c, NEP_EINVAL, "g is NULL");
+    c->grad_valid = true;
+    return h2d(c, c->g, g, 4 * (size_t)c->m.npar);
+}
+int nep_set_adam_state(nep_ctx* c, const float* m, const float* v, const float* vmax, int64_t t)
+{
+    CHECK_CTX(c);
+    if (!m || !v || !vmax || t < 0) return fail(c, NEP_EINVAL, "bad Adam state");
+    size_t nb = 4 * (size_t)c->m.npar;
+    int rc;
+    if ((rc = h2d(c, c->am, m, nb)) || (rc = h2d(c, c->av, v, nb)) || (rc = h2d(c, c->avmax, vmax, nb))) return rc;
+    c->t_adam = t;
+    return NEP_OK;
+}
+int nep_get_adam_state(nep_ctx* c, float* m, float* v, float* vmax, int64_t* t)
+{
+    CHECK_CTX(c);
+    size_t nb = 4 * (size_t)c->m.npar;
+    int rc;
+    if (m && (rc = d2h(c, m, c->am, nb))) return rc;
+    if (v && (rc = d2h(c, v, c->av, nb))) return rc;
+    if (vmax && (rc = d2h(c, vmax, c->avmax, nb))) return rc;
+    if (t) *t = c->t_adam;
+    return NEP_OK;
+}
+
+int nep_set_scaler(nep_ctx* c, const double* s)
+{
+    CHECK_CTX(c);
+    if (!s) return fail(c, NEP_EINVAL, "s is NULL");
+    std::vector<float> f(c->m.DP, 0.0f);
+    for (int i = 0; i < c->m.D; ++i) {
+        if (!std::isfinite(s[i])) return fail(c, NEP_EINVAL, "non-finite scaler");
+        f[i] = (float)s[i];
+    }
+    c->have_scaler = true; c->forward_valid = c->grad_valid = false;
+    return h2d(c, c->scaler, f.data(), 4 * f.size());
+}
+int nep_get_scaler(nep_ctx* c, double* s)
+{
+    CHECK_CTX(c);
+    if (!s) return fail(c, NEP_EINVAL, "s is NULL");
+    if (!c->have_scaler) return fail(c, NEP_ESTATE, "no scaler yet");
+    std::vector<float> f(c->m.DP);
+    int rc = d2h(c, f.data(), c->scaler, 4 * f.size());
+    if (rc) return rc;
+    for (int i = 0; i < c->m.D; ++i) s[i] = f[i];
+    return NEP_OK;
+}
+int nep_compute_scaler(nep_ctx* c)
+{
+    CHECK_CTX(c);
+    if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_compute_scaler before nep_build_neighbors");
+    if (!c->have_params) return fail(c, NEP_ESTATE, "nep_compute_scaler before nep_set_params");
+    int rc = nep_set_batch(c, 0, nullptr);
+    if (rc) return rc;
+    if ((rc = launch_forward(c, true))) return rc;
+    if ((rc = launch_scaler_minmax(c, c->scaler))) return rc;
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_scaler = true; c->forward_valid = c->grad_valid = false;
+    return NEP_OK;
+}
+
+static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs)
+{
+    BatchDev& b = c->b;
+    const ModelDev& m = c->m;
+    if (NBP > c->cap_NBP) {
+        void* olds[] = { b.q, b.Fp, b.h, b.S, b.Sd, b.qd, b.Qb, b.arow, b.Bd, b.F, b.u, b.Ei };
+        for (void* p : olds) dev_free(c, p);
+        size_t n = (size_t)NBP;
+        ALLOC(c, b.q, float, n * m.D);   ALLOC(c, b.Fp, float, n * m.D);  ALLOC(c, b.h, float, n * m.H);
+        ALLOC(c, b.S, float, n * m.nA * 24); ALLOC(c, b.Sd, float, n * m.nA * 24);
+        ALLOC(c, b.qd, float, n * m.D);  ALLOC(c, b.Qb, float, n * m.D);
+        ALLOC(c, b.arow, float, n * m.T * m.KRP); ALLOC(c, b.Bd, float, n * m.T * m.KR);
+        ALLOC(c, b.F, float, n * 3);     ALLOC(c, b.u, float, n * 3);     ALLOC(c, b.Ei, float, n);
+        c->cap_NBP = NBP;
+    }
+    if (Sb > c->cap_Sb) {
+        void* olds[] = { b.Es, b.Ws, b.eps, b.G, (void*)b.bsid, (void*)b.bnat, (void*)b.bfoff };
+        for (void* p : olds) dev_free(c, p);
+        ALLOC(c, b.Es, double, Sb); ALLOC(c, b.Ws, float, 9 * (size_t)Sb); ALLOC(c, b.eps, float, Sb); ALLOC(c, b.G, float, 9 * (size_t)Sb);
+        int* p1; int* p2; int64_t* p3;
+        ALLOC(c, p1, int, Sb); ALLOC(c, p2, int, Sb); ALLOC(c, p3, int64_t, Sb);
+        b.bsid = p1; b.bnat = p2; b.bfoff = p3;
+        c->cap_Sb = Sb;
+    }
+    if (nbs > c->cap_nbs) {
+        dev_free(c, (void*)b.bslice); dev_free(c, (void*)b.bsb); dev_free(c, (void*)b.bbase);
+        int *p1, *p2, *p3;
+        ALLOC(c, p1, int, nbs); ALLOC(c, p2, int, nbs); ALLOC(c, p3, int, nbs);
+        b.bslice = p1; b.bsb = p2; b.bbase = p3;
+        c->cap_nbs = nbs;
+    }
+    if (!b.lacc) ALLOC(c, b.lacc, double, 8);
+    return NEP_OK;
+}
+
+int nep_set_batch(nep_ctx* c, int n, const int* ids)
+{
+    CHECK_CTX(c);
+    if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_set_batch before nep_build_neighbors");
+    if (ids && n < 0) return fail(c, NEP_EINVAL, "negative batch size");
+    int Sb = ids ? n : c->S;
+    std::vector<int> bsid(Sb), bnat(Sb), bslice, bsb, bbase;
+    std::vector<int64_t> bfoff(Sb);
+    std::vector<unsigned char> seen(ids ? c->S : 0, 0);
+    int64_t Nb = 0, nbp = 0, PRb = 0, PAb = 0;
+    int Sv = 0;
+    for (int k = 0; k < Sb; ++k) {
+        int s = ids ? ids[k] : k;
+        if (s < 0 || s >= c->S) return fail(c, NEP_EINVAL, "structure id out of range");
+        if (ids) { if (seen[s]) return fail(c, NEP_EINVAL, "duplicate structure id in batch"); seen[s] = 1; }
+        bsid[k] = s; bnat[k] = c->h_nat[s]; bfoff[k] = Nb;
+        Nb += c->h_nat[s];
+        Sv += c->h_hasv.empty() ? 1 : c->h_hasv[s];
+        PRb += c->h_pairsR_struct[s]; PAb += c->h_pairsA_struct[s];
+        for (int64_t sl = c->h_pbase[s] / WARP; sl < c->h_pbase[s + 1] / WARP; ++sl) {
+            bslice.push_back((int)sl); bsb.push_back(k); bbase.push_back((int)nbp);
+        }
+        nbp += c->h_pbase[s + 1] - c->h_pbase[s];
+        if (nbp > INT32_MAX / 2) return fail(c, NEP_ECAPACITY, "batch too large");
+    }
+    int nbs = (int)bslice.size();
+    int rc = ensure_batch_capacity(c, std::max<int64_t>(nbp, WARP), std::max(Sb, 1), std::max(nbs, 1));
+    if (rc) return rc;
+    BatchDev& b = c->b;
+    b.Sb = Sb; b.Sv = Sv; b.Nb = Nb; b.nbs = nbs; b.NBP = nbp;
+    if (Sb) {
+        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bsid, bsid.data(), 4 * (size_t)Sb, cudaMemcpyHostToDevice, c->stream));
+        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bnat, bnat.data(), 4 * (size_t)Sb, cudaMemcpyHostToDevice, c->stream));
+        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bfoff, bfoff.data(), 8 * (size_t)Sb, cudaMemcpyHostToDevice, c->stream));
+        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bslice, bslice.data(), 4 * (size_t)nbs, cudaMemcpyHostToDevice, c->stream));
+        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bsb, bsb.data(), 4 * (size_t)nbs, cudaMemcpyHostToDevice, c->stream));
+        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bbase, bbase.data(), 4 * (size_t)nbs, cudaMemcpyHostToDevice, c->stream));
+        NEP_CUDA(c, cudaStreamSynchronize(c->stream));   // host vectors die at return
+    }
+    c->h_bsid = bsid; c->h_bfoff = bfoff; c->PRb = PRb; c->PAb = PAb;
+    c->forward_valid = c->grad_valid = false;
+    return NEP_OK;
+}
+
+static int copy_out(nep_ctx* c, void* dst, const float* src, size_t count, int on_host)
+{
+    if (!dst || !count) return NEP_OK;
+    NEP_CUDA(c, cudaMemcpyAsync(dst, src, 4 * count, on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
+    return NEP_OK;
+}
+
+int nep_forward(nep_ctx* c, void* E_out, void* F_out, void* W_out, int on_host)
+{
+    CHECK_CTX(c);
+    if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_forward before nep_build_neighbors");
+    if (!c->have_params) return fail(c, NEP_ESTATE, "nep_forward before nep_set_params");
+    if (!c->have_scaler) return fail(c, NEP_ESTATE, "nep_forward before nep_set_scaler / nep_compute_scaler");
+    int rc = launch_forward(c, false);
+    if (rc) return rc;
+    c->forward_valid = true; c->grad_valid = false;
+    if (E_out || F_out || W_out) {
+        const BatchDev& b = c->b;
+        size_t nE = (size_t)b.Sb, nF = 3 * (size_t)b.Nb, nW = 9 * (size_t)b.Sb;
+        if (on_host) {
+            float* stage = (float*)dev_alloc(c, 4 * (nE + nF + nW + 1));
+            if (!stage) return NEP_ENOMEM;
+            rc = launch_gather_outputs(c, E_out ? stage : nullptr, F_out ? stage + nE : nullptr, W_out ? stage + nE + nF : nullptr);
+            if (!rc) rc = copy_out(c, E_out, stage, nE, 1);
+            if (!rc) rc = copy_out(c, F_out, stage + nE, nF, 1);
+            if (!rc) rc = copy_out(c, W_out, stage + nE + nF, nW, 1);
+            cudaError_t e = cudaStreamSynchronize(c->stream);
+            dev_free(c, stage);
+            if (rc) return rc;
+            if (e != cudaSuccess) return fail(c, NEP_ECUDA, std::string("nep_forward: ") + cudaGetErrorString(e));
+        } else {
+            if ((rc = launch_gather_outputs(c, (float*)E_out, (float*)F_out, (float*)W_out))) return rc;
+        }
+    }
+    return NEP_OK;
+}
+
+int nep_get_descriptors(nep_ctx* c, float* q)
+{
+    CHECK_CTX(c);
+    if (!q) return fail(c, NEP_EINVAL, "q is NULL");
+    if (!c->forward_valid) return fail(c, NEP_ESTATE, "nep_get_descriptors needs nep_forward first");
+    size_t n = (size_t)c->b.Nb * c->m.D;
+    float* stage = (float*)dev_alloc(c, 4 * std::max<size_t>(n, 1));
+    if (!stage) return NEP_ENOMEM;
+    int rc = launch_gather_q(c, stage);
+    if (!rc) rc = d2h(c, q, stage, 4 * n);
+    dev_free(c, stage);
+    return rc;
+}
+
+int nep_get_loss(nep_ctx* c, double* loss4)
+{
+    CHECK_CTX(c);
+    if (!loss4) return fail(c, NEP_EINVAL, "loss4 is NULL");
+    if (!c->grad_valid) return fail(c, NEP_ESTATE, "nep_get_loss needs nep_loss_grad first");
+    return d2h(c, loss4, c->b.lacc + 4, 32);
+}
+
+int nep_loss_grad(nep_ctx* c, double lambda_E, double lambda_F, double lambda_V, double* loss4_host)
+{
+    CHECK_CTX(c);
+    if (!c->forward_valid) return fail(c, NEP_ESTATE, "nep_loss_grad needs nep_forward on the same batch and parameters first");
+    if (!c->have_labels) return fail(c, NEP_ESTATE, "nep_loss_grad needs labels (nep_load_structures / nep_set_labels)");
+    if (!(lambda_E >= 0) || !(lambda_F >= 0) || !(lambda_V >= 0)) return fail(c, NEP_EINVAL, "loss weights must be >= 0");
+    c->lamE = lambda_E; c->lamF = lambda_F; c->lamV = lambda_V;
+    int rc = launch_loss_grad(c);
+    if (rc) return rc;
+    c->grad_valid = true;
+    if (loss4_host) return d2h(c, loss4_host, c->b.lacc + 4, 32);
+    return NEP_OK;
+}
+
+int nep_adam_step(nep_ctx* c, double lr, double beta1, double beta2, double eps, int variant)
+{
+    CHECK_CTX(c);
+    if (!c->grad_valid) return fail(c, NEP_ESTATE, "nep_adam_step needs a gradient (nep_loss_grad)");
+    if (!(lr >= 0) || !(beta1 >= 0 && beta1 < 1) || !(beta2 >= 0 && beta2 < 1) || !(eps >= 0) || (variant != 0 && variant != 1))
+        return fail(c, NEP_EINVAL, "bad Adam hyper-parameter");
+    int rc = launch_adam(c, lr, beta1, beta2, eps, variant);
+    if (rc) return rc;
+    c->forward_valid = false; c->grad_valid = false;
+    return NEP_OK;
+}
+
+int nep_synchronize(nep_ctx* c)
+{
+    CHECK_CTX(c);
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NEP_OK;
+}
+
+int nep_launch_count(nep_ctx* c, int64_t* n)
+{
+    CHECK_CTX(c);
+    if (n) *n = c->launches;
+    return NEP_OK;
+}
+int nep_profile_enable(nep_ctx* c, int on)
+{
+    CHECK_CTX(c);
+    cudaStreamSynchronize(c->stream);
+    for (auto& r : c->prof.pending) { c->prof.pool.push_back(r.a); c->prof.pool.push_back(r.b); }
+    c->prof.pending.clear(); c->prof.acc.clear();
+    c->prof.on = on != 0;
+    return NEP_OK;
+}
+int nep_profile_read(nep_ctx* c, int cap, const char** names, double* ms, int64_t* launches, int* n)
+{
+    CHECK_CTX(c);
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    static thread_local std::vector<std::string> keep;
+    for (auto& r : c->prof.pending) {
+        float t = 0.f;
+        cudaEventElapsedTime(&t, r.a, r.b);
+        auto& a = c->prof.acc[r.name];
+        a.first += t; a.second += 1;
+        c->prof.pool.push_back(r.a); c->prof.pool.push_back(r.b);
+    }
+    c->prof.pending.clear();
+    keep.clear();
+    int k = 0;
+    for (auto& kv : c->prof.acc) keep.push_back(kv.first);
+    for (auto& kv : c->prof.acc) {
+        if (k >= cap) break;
+        if (names) names[k] = keep[k].c_str();
+        if (ms) ms[k] = kv.second.first;
+        if (launches) launches[k] = kv.second.second;
+        ++k;
+    }
+    if (n) *n = k;
+    c->prof.acc.clear();
+    return NEP_OK;
+}
+
+int nep_get_sizes(nep_ctx* c, int64_t* s)
+{
+    CHECK_CTX(c);
+    if (!s) return fail(c, NEP_EINVAL, "sizes8 is NULL");
+    s[0] = c->S; s[1] = c->N; s[2] = c->PR; s[3] = c->PA; s[4] = c->b.Sb; s[5] = c->b.Nb; s[6] = c->PRb; s[7] = c->PAb;
+    return NEP_OK;
+}
+
+}  // extern "C"

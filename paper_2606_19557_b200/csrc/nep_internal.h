@@ -1,0 +1,156 @@
+// nep_internal.h -- context, device views and launcher declarations shared by the .cu files of libnep_b200.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/nep.h"
+
+namespace nep {
+
+constexpr int WARP = 32;
+constexpr int MAX_T = 16;
+constexpr int MAX_NCH = 5;   // angular channels held in registers by one thread
+
+// Everything a kernel needs to know about the model (passed by value).
+struct ModelDev {
+    int T, nR, nA, KR, KA, KRP, H, HP, D, DP, nang, has4, has5;   // HP, DP: H, D padded to multiples of 8
+    float rcR, rcA, rcinvR, rcinvA;
+    // offsets into theta
+    int per_type;          // (D + 2) * H
+    int o_b1, o_cR, o_cA;
+    int npar;
+};
+
+// Resident data set (positions fixed for the whole training run).
+struct DataDev {
+    int S;                 // structures
+    int64_t N;             // atoms
+    int64_t NP;            // padded atoms: every structure padded to a multiple of 32 (one warp = one slice)
+    int nslices;           // NP / 32
+    const double* pos;     // [N][3]
+    const double* box;     // [S][9]
+    const int* type;       // [N]
+    const int64_t* atom_off;   // [S+1]
+    const int64_t* pbase;      // [S+1] padded offset of each structure
+    const int* type_p;     // [NP], -1 = padding
+    const int* slice_struct;   // [nslices]
+    // labels
+    const double* Elab;    // [S]
+    const float* Flab;     // [3][NP]
+    const float* Wlab;     // [S][9]
+    const unsigned char* hasv; // [S]
+    // canonical neighbour lists (CSR over the N atoms)
+    const int64_t* offR; const int* jR; const signed char* shR;
+    const int64_t* offA; const int* jA; const signed char* shA;
+    // sliced pair cache: record (slice, slot s, lane) at rec[recoff[slice] + s*32 + lane]
+    const int* cntR; const int64_t* recoffR; const float4* recR;
+    const int* cntA; const int64_t* recoffA; const float4* recA;
+    const float* B;        // [T*KR][NP] radial aggregate  B_k[T'] = sum_{j in N_R(i), t_j = T'} f_k(r_ij)
+};
+
+// Current mini-batch: a list of slices, all per-step temporaries are indexed by batch-padded atom ib = w*32 + lane.
+struct BatchDev {
+    int Sb;                // structures in the batch
+    int Sv;                // ... of which have virial labels
+    int64_t Nb;            // atoms in the batch
+    int nbs;               // slices in the batch
+    int64_t NBP;           // nbs * 32
+    const int* bslice;     // [nbs] data-set slice id
+    const int* bsb;        // [nbs] batch structure index of the slice
+    const int* bbase;      // [nbs] batch-padded index of the first atom of the slice's structure
+    const int* bsid;       // [Sb]  data-set structure id
+    const int* bnat;       // [Sb]  atoms of the structure
+    const int64_t* bfoff;  // [Sb]  first atom in batch order (unpadded), for outputs
+    // temporaries
+    float* q;      // [D][NBP]   unscaled descriptors
+    float* Fp;     // [D][NBP]   dE_i/dq
+    float* h;      // [H][NBP]   tanh
+    float* S;      // [nA*24][NBP] normalised angular moments
+    float* Sd;     // [nA*24][NBP] their tangent
+    float* qd;     // [D][NBP]   tangent of q (angular part written by the tangent sweep, radial by the network kernel)
+    float* Qb;     // [D][NBP]   adjoint of q
+    float* arow;   // [NBP][T][KRP]  a_k[T'] = sum_n Fp_n cR[t_i][T'][n][k]
+    float* Bd;     // [T*KR][NBP] tangent of B
+    float* F;      // [3][NBP]
+    float* u;      // [3][NBP]   dL/dF
+    float* Ei;     // [NBP]
+    double* Es;    // [Sb]
+    float* Ws;     // [Sb][9]
+    float* eps;    // [Sb]       dL/dE_s
+    float* G;      // [Sb][9]    dL/dW_s
+    double* lacc;  // [4] sums: (dE)^2, |dF|^2, (dW)^2, spare ; loss4 at [4..7]
+};
+
+struct Profiler {
+    bool on = false;
+    struct Rec { cudaEvent_t a, b; const char* name; };
+    std::vector<Rec> pending;
+    std::map<std::string, std::pair<double, int64_t>> acc;
+    std::vector<cudaEvent_t> pool;
+};
+
+}  // namespace nep
+
+struct nep_ctx {
+    nep::ModelDev m;
+    double rcR, rcA;
+    int n_max_R, n_max_A, basis_R, basis_A, l3, l4, l5;
+    nep_alloc_fn alloc; nep_free_fn free_; void* user;
+    cudaStream_t stream;
+    std::string err;
+    std::vector<void*> allocs;
+    int sm_count; int max_smem_optin;
+
+    // host copies of the data set
+    int S = 0; int64_t N = 0, NP = 0; int nslices = 0;
+    std::vector<int> h_nat; std::vector<int64_t> h_aoff, h_pbase; std::vector<unsigned char> h_hasv;
+    std::vector<double> h_box;
+    bool have_data = false, have_labels = false, have_nbrs = false, have_params = false, have_scaler = false;
+    bool forward_valid = false, grad_valid = false;
+    int64_t PR = 0, PA = 0;
+
+    nep::DataDev d{};
+    nep::BatchDev b{};
+    int64_t cap_NBP = 0; int cap_Sb = 0; int cap_nbs = 0;
+    std::vector<int> h_bsid; std::vector<int64_t> h_bfoff;
+    int64_t PRb = 0, PAb = 0;
+    std::vector<int64_t> h_pairsR_struct, h_pairsA_struct;   // pairs per structure (for sizes / flop models)
+
+    float *theta = nullptr, *g = nullptr, *am = nullptr, *av = nullptr, *avmax = nullptr, *scaler = nullptr;
+    int64_t t_adam = 0;
+    double lamE = 0, lamF = 0, lamV = 0;
+
+    int64_t launches = 0;
+    nep::Profiler prof;
+};
+
+namespace nep {
+
+// ---- helpers implemented in nep_api.cu ----
+int fail(nep_ctx* c, int code, const std::string& msg);
+void* dev_alloc(nep_ctx* c, size_t bytes);        // nullptr on failure (err set)
+void dev_free(nep_ctx* c, void* p);
+void prof_begin(nep_ctx* c, const char* name);
+void prof_end(nep_ctx* c);
+
+#define NEP_CUDA(c, expr)                                                                     \
+    do {                                                                                      \
+        cudaError_t e__ = (expr);                                                             \
+        if (e__ != cudaSuccess)                                                               \
+            return nep::fail((c), NEP_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e__)); \
+    } while (0)
+
+// ---- launchers (each returns NEP_OK or an error code with c->err set) ----
+int build_neighbors_dev(nep_ctx* c);                           // nep_neighbor.cu : S0a + S0b
+int launch_forward(nep_ctx* c, bool descriptors_only);         // nep_forward.cu  : S1-S5
+int launch_loss_grad(nep_ctx* c);                              // nep_backward.cu : S6-S9
+int launch_adam(nep_ctx* c, double lr, double b1, double b2, double eps, int variant);  // nep_adam.cu : S10
+int launch_scaler_minmax(nep_ctx* c, float* d_s);              // nep_forward.cu  : S0c (after a descriptors-only pass over all)
+int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW);  // nep_forward.cu: batch-padded -> batch order
+int launch_gather_q(nep_ctx* c, float* dq);                    // [N_b][D]
+
+}  // namespace nep
