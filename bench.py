@@ -1,0 +1,424 @@
+#!/usr/bin/env python
+"""bench.py -- NEP training-step throughput (atoms/s) on B200, BASELINE.json's metric.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+nep_forward (descriptors, network, E, F, virial) + nep_loss_grad (loss, every gradient) + nep_adam_step.
+N = 1 workload: BASELINE.json configs[1] (1000 bcc structures x 128 atoms, full NEP4 descriptor, batch 1000).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--n-struct S]
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 9 for the keys and the flop / byte models of `roofline`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "NEP training-step throughput (atoms/s, E+F+virial loss+grads+Adam)"
+UNIT = "atoms/s"
+LR = 1e-3
+FP32_LANES_PER_SM = 128          # B300_MICROARCH / blackwell guide: 4 SMSPs x 32 FP32 lanes
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config id (1..5); 2 is the headline workload")
+    ap.add_argument("--n-struct", type=int, default=None, help="use only the first S structures (debugging; not a bench line)")
+    ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--model-index", type=int, default=0, help="config 5: which of the 8 sweep models")
+    return ap.parse_args()
+
+
+def make_workload(args, rank: int = 0):
+    from paper_2606_19557_b200 import workloads as wl
+    model = wl.config5_sweep()[args.model_index] if args.config == 5 else None
+    return wl.make_config(args.config, n_struct=args.n_struct, model=model)
+
+
+def workload_name(w, args):
+    m = w.model
+    return (f"config{w.config_id}: {w.name}; {w.structures.n_struct} structures, batch {w.batch_size}; "
+            f"T={m.n_species} rc={m.rc_R}/{m.rc_A} n_max={m.n_max_R}/{m.n_max_A} basis={m.basis_R}/{m.basis_A} "
+            f"l_max=({m.l_max_3b},{m.l_max_4b},{m.l_max_5b}) neurons={m.neurons} D={m.D} N_par={m.n_par}")
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# clocks
+# ----------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int = 0, period_ms: int = 100):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", str(period_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for r in self.rows if t0 - 0.05 <= r[0] <= t1 + 0.25] or self.rows
+        for _, line in rows:
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# problem set-up on the GPU (input recipe of DESIGN.md section 5; everything computed by the library itself)
+# ----------------------------------------------------------------------------------------------------------------
+def draw_theta(nep, model, seed):
+    """ParamDraw two-phase recipe with the descriptors / scaler computed by the CUDA library (the implementation under test)."""
+    from paper_2606_19557_b200.workloads import ParamDraw
+    pd = ParamDraw(model, seed)
+    nep.set_params(pd.coefficients().astype(np.float32))
+    nep.compute_scaler()                       # Eq. 2 at these coefficients, over every loaded atom
+    s = nep.get_scaler()
+    nep.forward(want=())
+    q = nep.get_descriptors().astype(np.float64)
+    theta = pd.network((q * s).mean(axis=0)).astype(np.float32)
+    return theta, s
+
+
+def setup_ours(w, stream=None):
+    from paper_2606_19557_b200.binding import Nep
+    import torch
+    t0 = time.time()
+    nep = Nep.from_model(w.model, stream=stream)
+    st = w.structures
+    nep.load_structure_set(st)
+    t1 = time.time()
+    nep.build_neighbors()
+    nep.synchronize()
+    t2 = time.time()
+    th_t, s_t = draw_theta(nep, w.model, w.seeds["teacher"])
+    nep.set_params(th_t); nep.set_scaler(s_t)
+    E, F, W = nep.forward()                    # teacher labels (they set the values being fitted, not the work)
+    nep.set_labels(E.astype(np.float64), F.astype(np.float64), W.astype(np.float64))
+    th_s, s_s = draw_theta(nep, w.model, w.seeds["student"])
+    nep.set_params(th_s); nep.set_scaler(s_s)
+    nep.set_batch(None)
+    torch.cuda.synchronize()
+    return nep, dict(load_s=t1 - t0, neighbors_cache_s=t2 - t1, params_labels_s=time.time() - t2)
+
+
+def one_step(nep, lam):
+    nep.forward_device()
+    nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
+    nep.adam_step(LR)
+
+
+def e2e_step(nep, lam, ids):
+    """The call sequence a user makes per training step, HOST buffers in and out: the batch's structure ids go in
+    (nep_set_batch copies them and the slice tables to the device), the loss comes back (nep_loss_grad -> host)."""
+    nep.set_batch(ids)
+    nep.forward_device()
+    l4 = nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=True)
+    nep.adam_step(LR)
+    return l4
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the NEP step has no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_19557_b200 import workloads as wl, roofline as rf
+    from paper_2606_19557_b200 import build as nbuild
+    if rank == 0:
+        nbuild.build()
+    if world > 1:
+        dist.barrier()
+    w = make_workload(args, rank)
+    nep, setup = setup_ours(w)
+    lam = w.lambdas
+    blist = wl.batches(w)
+    full_batches = [b for b in blist if len(b) == w.batch_size] or blist
+    single = len(blist) == 1
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+    hbm_peak = peaks["hbm_gbs"] if peaks else 6650.0
+    peak_src = "measured (MEASURED_PEAKS.json)" if peaks else "fallback (B200_PROFILING.md)"
+
+    flush = None if args.no_flush else torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # 2x the 126 MB L2
+
+    def set_b(i):
+        if not single:
+            nep.set_batch(full_batches[i % len(full_batches)])
+
+    # ---- warm-up ----
+    if single:
+        nep.set_batch(None)
+    for i in range(max(args.warmup, 3)):
+        set_b(i); one_step(nep, lam)
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, CUDA events per step on the launching stream, L2 flushed between steps ----
+    K = args.steps
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    atoms = structs = 0
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(local) if rank == 0 else None
+    nep.profile_enable(True)
+    l0 = nep.launch_count()
+    t0 = time.time()
+    for i in range(K):
+        set_b(i)
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        sz = nep.batch_shape()
+        structs += sz[0]; atoms += sz[1]
+        ev[i][0].record()
+        one_step(nep, lam)
+        ev[i][1].record()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    if world > 1:
+        dist.barrier()
+    launches = nep.launch_count() - l0
+    prof = nep.profile_read()
+    nep.profile_enable(False)
+    clk = clocks.stop(t0, t1) if clocks else None
+    ms_steps = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(ms_steps))
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        c = torch.tensor([atoms, structs], device="cuda", dtype=torch.float64)
+        dist.all_reduce(c)
+        atoms, structs = int(c[0].item()), int(c[1].item())
+    value = atoms / (total_ms * 1e-3)
+
+    # ---- back-to-back (no flush, no per-kernel events), for transparency ----
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for i in range(K):
+        set_b(i); one_step(nep, lam)
+    b.record(); torch.cuda.synchronize()
+    ms_b2b = a.elapsed_time(b) / K
+
+    # ---- e2e: host ids in, host loss out, every step ----
+    e2e_batches = full_batches if not single else [np.arange(w.structures.n_struct, dtype=np.int32)]
+    for i in range(3):
+        e2e_step(nep, lam, e2e_batches[i % len(e2e_batches)])
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    e_atoms = 0
+    h2d = d2h = 0
+    te0 = time.perf_counter()
+    a.record()
+    for i in range(K):
+        ids = e2e_batches[i % len(e2e_batches)]
+        l4 = e2e_step(nep, lam, ids)
+        Sb, Nb = nep.batch_shape()
+        e_atoms += Nb
+        nbs = int(np.sum((w.structures.n_atoms[ids] + 31) // 32))
+        h2d += Sb * 16 + nbs * 12
+        d2h += 32
+    b.record(); torch.cuda.synchronize()
+    e2e_ms = max(a.elapsed_time(b), (time.perf_counter() - te0) * 1e3)   # host-side work (tables) is part of the call
+    if world > 1:
+        t = torch.tensor([e2e_ms, 0.0], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t[0].item())
+        c = torch.tensor([e_atoms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(c)
+        e_atoms = int(c.item())
+    e2e_value = e_atoms / (e2e_ms * 1e-3)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- roofline of the dominant kernel ----
+    if single:
+        nep.set_batch(None)
+    else:
+        nep.set_batch(full_batches[0])
+    sizes = nep.get_sizes()
+    models = rf.kernel_models(w.model, sizes)
+    ksum = sum(v[0] for v in prof.values())
+    kern = {k: {"ms": v[0] / max(v[1], 1), "launches_per_step": v[1] / K, "share": v[0] / ksum} for k, v in prof.items()}
+    top = max(kern, key=lambda k: kern[k]["share"])
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    alu_peak = rf.fp32_peak_flops(sm_count, (clk or {}).get("sm_max_mhz") or 1965.0, FP32_LANES_PER_SM)
+    mdl = models.get(top)
+    roof = None
+    if mdl:
+        dur = kern[top]["ms"] * 1e-3
+        t_alu, t_hbm = mdl["flops"] / alu_peak, mdl["bytes"] / (hbm_peak * 1e9)
+        if t_alu >= t_hbm:
+            roof = {"kernel": top, "bound": "alu", "achieved": mdl["flops"] / dur / 1e12, "peak": alu_peak / 1e12, "unit": "TFLOP/s",
+                    "peak_source": f"derived: {sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (DESIGN.md section 9)"}
+        else:
+            roof = {"kernel": top, "bound": "hbm", "achieved": mdl["bytes"] / dur / 1e9, "peak": hbm_peak, "unit": "GB/s", "peak_source": peak_src}
+        roof["frac"] = roof["achieved"] / roof["peak"]
+        roof["traffic"] = None
+        roof["share_of_step"] = kern[top]["share"]
+        roof["avg_ms"] = kern[top]["ms"]
+        roof["algorithmic_flops_per_launch"] = mdl["flops"]
+        roof["algorithmic_bytes_per_launch"] = mdl["bytes"]
+    tot = rf.step_totals(models)
+    ms_step = total_ms / K
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic (seeded lattices, teacher-NEP labels; stand-in for the paper's DFT sets)",
+        "config": {"workload": workload_name(w, args), "structures_per_s": structs / (total_ms * 1e-3),
+                   "atoms_per_step": atoms // K // world, "pairs_R_per_step": sizes["P_R_b"], "pairs_A_per_step": sizes["P_A_b"],
+                   "l2": ("flushed between timed steps (256 MB write)" if flush is not None else "not flushed; per-step working set exceeds L2"),
+                   "ms_per_step_back_to_back_no_flush": ms_b2b, "setup_s": setup,
+                   "device_bytes": nep.bytes_allocated, "parallelism": f"dp{world} (structures sharded, no data-path collective)"},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
+                "what": "per step: nep_set_batch(host ids) + nep_forward + nep_loss_grad(loss -> host) + nep_adam_step; geometry cache resident (P:143)"},
+        "gpu_launches": int(launches),
+        "clocks": clk,
+        "roofline": roof,
+        "kernels": {k: {"avg_ms": round(v["ms"], 5), "share": round(v["share"], 4), "per_step": v["launches_per_step"]} for k, v in
+                    sorted(kern.items(), key=lambda kv: -kv[1]["share"])},
+        "step_model": {"flops": tot["flops"], "bytes": tot["bytes"], "alu_frac_of_step": tot["flops"] / alu_peak / (ms_step * 1e-3),
+                       "hbm_frac_of_step": tot["bytes"] / (hbm_peak * 1e9) / (ms_step * 1e-3)},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        out["cpu_baseline"] = cpu_baseline(args, w, seconds_target=15.0)
+    nep.destroy()
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# the oracle on the host cores: cpu_baseline leg and --impl reference arm (the only places bench.py executes oracle/)
+# ----------------------------------------------------------------------------------------------------------------
+def oracle_problem(w, n_sample):
+    """First n_sample structures of the workload, teacher labels and student parameters, all from the oracle."""
+    import dataclasses
+    from oracle.problem import make_problem
+    st = w.structures.subset(list(range(min(n_sample, w.structures.n_struct))))
+    ws = dataclasses.replace(w, structures=st, batch_size=min(w.batch_size, st.n_struct))
+    return make_problem(ws)
+
+
+def oracle_step(O, prob, state, lam):
+    th, m, v, vm = state["theta"], state["m"], state["v"], state["vmax"]
+    l4, g = O.loss_grad(prob.data, th, prob.scaler, lam)      # forward E/F/W + loss + every gradient (C7-C12)
+    state["t"] = O.adam_step(th, g, m, v, vm, state["t"], LR)  # C13
+    return l4
+
+
+def cpu_baseline(args, w, seconds_target=15.0):
+    from oracle import nep_oracle as O
+    cores = O.max_threads()
+    n = min(w.structures.n_struct, 32)
+    prob = oracle_problem(w, n)
+    npar = w.model.n_par
+    state = dict(theta=prob.theta.copy(), m=np.zeros(npar), v=np.zeros(npar), vmax=np.zeros(npar), t=0)
+    oracle_step(O, prob, state, w.lambdas)
+    t0 = time.perf_counter(); oracle_step(O, prob, state, w.lambdas); dt = time.perf_counter() - t0
+    atoms = int(prob.workload.structures.n_atoms.sum())
+    # scale the sample so that 3 timed steps take about seconds_target
+    want = int(max(n, min(w.structures.n_struct, n * seconds_target / 3.0 / max(dt, 1e-4))))
+    if want > n:
+        prob = oracle_problem(w, want)
+        state = dict(theta=prob.theta.copy(), m=np.zeros(npar), v=np.zeros(npar), vmax=np.zeros(npar), t=0)
+        atoms = int(prob.workload.structures.n_atoms.sum())
+        oracle_step(O, prob, state, w.lambdas)
+    best = 1e30
+    for _ in range(3):
+        t0 = time.perf_counter(); oracle_step(O, prob, state, w.lambdas); best = min(best, time.perf_counter() - t0)
+    return {"value": atoms / best, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {prob.workload.structures.n_struct} structures ({atoms} atoms) of the workload, one full step "
+                      f"(fp64 forward + loss + gradient + Adam), best of 3, OpenMP over structures"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank != 0:
+        return
+    from oracle import nep_oracle as O
+    w = make_workload(args)
+    n = min(w.structures.n_struct, 128)        # bounded sample per step: the whole run stays within a few minutes
+    prob = oracle_problem(w, n)
+    npar = w.model.n_par
+    state = dict(theta=prob.theta.copy(), m=np.zeros(npar), v=np.zeros(npar), vmax=np.zeros(npar), t=0)
+    atoms = int(prob.workload.structures.n_atoms.sum())
+    W = max(args.warmup, 1)
+    for _ in range(W):
+        oracle_step(O, prob, state, w.lambdas)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(O, prob, state, w.lambdas)
+    dt = time.perf_counter() - t0
+    value = atoms * args.steps / dt
+    sample = f"first {n} structures ({atoms} atoms) of the workload per step"
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+           "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic (seeded lattices, teacher-NEP labels)",
+           "config": {"workload": workload_name(w, args), "sample": sample},
+           "cpu_baseline": {"value": value, "unit": UNIT, "kind": "oracle", "cores": O.max_threads(), "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

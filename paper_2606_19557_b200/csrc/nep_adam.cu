@@ -10,13 +10,13 @@ namespace nep {
 template <int VARIANT>
 __global__ void __launch_bounds__(256) k_adam(int n, float* __restrict__ theta, const float* __restrict__ g, float* __restrict__ m,
                                               float* __restrict__ v, float* __restrict__ vmax, float lr, float beta1, float beta2,
-                                              float eps, float inv_bc1, float inv_bc2)
+                                              float omb1, float omb2, float eps, float inv_bc1, float inv_bc2)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float gi = g[i];
-    const float mi = fmaf(beta1, m[i], (1.0f - beta1) * gi);          // Eq. 9
-    const float vi = fmaf(beta2, v[i], (1.0f - beta2) * gi * gi);     // Eq. 10
+    const float mi = fmaf(beta1, m[i], omb1 * gi);                      // Eq. 9 (omb = 1 - beta rounded from fp64)
+    const float vi = fmaf(beta2, v[i], omb2 * gi * gi);                 // Eq. 10
     m[i] = mi; v[i] = vi;
     const float mh = mi * inv_bc1;                                    // Eq. 11
     if (VARIANT == 0) {
@@ -39,10 +39,10 @@ int launch_adam(nep_ctx* c, double lr, double b1, double b2, double eps, int var
     const unsigned grid = (unsigned)((n + 255) / 256);
     if (variant == 0)
         NEP_LAUNCH(c, "k_adam", k_adam<0>, grid, 256, 0, n, c->theta, c->g, c->am, c->av, c->avmax, (float)lr, (float)b1, (float)b2,
-                   (float)eps, (float)(1.0 / bc1), (float)(1.0 / bc2));
+                   (float)(1.0 - b1), (float)(1.0 - b2), (float)eps, (float)(1.0 / bc1), (float)(1.0 / bc2));
     else
         NEP_LAUNCH(c, "k_adam", k_adam<1>, grid, 256, 0, n, c->theta, c->g, c->am, c->av, c->avmax, (float)lr, (float)b1, (float)b2,
-                   (float)eps, (float)(1.0 / bc1), (float)(1.0 / bc2));
+                   (float)(1.0 - b1), (float)(1.0 - b2), (float)eps, (float)(1.0 / bc1), (float)(1.0 / bc2));
     return NEP_OK;
 }
 

@@ -1,0 +1,222 @@
+"""GPU parity: libnep_b200 (through the C ABI binding) against the fp64 oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: neighbour lists bit-exact; E <= 1e-5 eV/atom; F, W <= 1e-4 relative in
+norm; gradient <= 1e-3 relative in norm.  Sizes: several 32-atom slices plus ragged tails, multi-image boxes."""
+import numpy as np
+import pytest
+
+from oracle import nep_oracle as O
+from paper_2606_19557_b200 import workloads as wl
+from tests import _gpu_harness as H
+
+pytestmark = pytest.mark.gpu
+
+
+def _cases():
+    m5 = wl.config5_sweep()
+    return {
+        "tiny_T2": lambda: wl.tiny_workload(0),
+        "tiny_T1": lambda: wl.tiny_workload(1, n_species=1, sizes=(3, 9, 1), box=(3.0, 4.0, 2.9)),
+        "tiny_T3_ragged": lambda: wl.tiny_workload(2, n_species=3, sizes=(33, 2, 40), box=(7.5, 3.1, 8.0)),
+        "tiny_thin_boxes": lambda: wl.tiny_workload(7, n_species=2, sizes=(1, 2, 3), box=(1.6, 2.2, 2.0)),   # images up to +-2
+        "tiny_3body_only": lambda: wl.tiny_workload(3, model=wl.ModelSpec(2, 3.2, 2.6, 2, 0, 3, 1, 4, 0, 0, 5)),
+        "tiny_4body_only": lambda: wl.tiny_workload(4, model=wl.ModelSpec(2, 3.2, 3.2, 0, 2, 1, 3, 4, 2, 0, 3)),
+        "tiny_5body_only": lambda: wl.tiny_workload(5, model=wl.ModelSpec(2, 3.0, 2.0, 1, 1, 2, 2, 4, 0, 1, 9)),
+        "cfg1a": lambda: wl.make_config(1),
+        "cfg1b": lambda: wl.make_config(1, n_struct=2, variant="1b"),
+        "cfg2": lambda: wl.make_config(2, n_struct=6),
+        "cfg3": lambda: wl.make_config(3, n_struct=8),
+        "cfg4": lambda: wl.make_config(4, n_struct=12),
+        "cfg5_small_model": lambda: wl.make_config(5, n_struct=8),
+        "cfg5_large_model": lambda: wl.make_config(5, n_struct=8, model=m5[-1]),      # n_max 8, basis 12, 100 neurons
+        "cfg5_mixed_model": lambda: wl.make_config(5, n_struct=6, model=m5[5]),       # n_max 8, basis 8, 100 neurons
+        "wide_T16": lambda: wl.tiny_workload(6, n_species=16, sizes=(40, 37), box=(7.0, 6.5),
+                                             model=wl.ModelSpec(16, 3.2, 2.6, 3, 3, 4, 4, 4, 2, 1, 12)),
+    }
+
+
+CASES = _cases()
+_cache = {}
+
+
+def _prob(name):
+    if name not in _cache:
+        _cache[name] = H.make_problem(CASES[name]())
+    return _cache[name]
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_neighbor_lists_bit_exact(name):
+    prob = _prob(name)
+    with H.make_gpu(prob, labels=False, scaler=None) as nep:
+        H.check_neighbors(nep, prob.data)
+        s = nep.get_sizes()
+        assert s["P_R"] == len(prob.data.jR) and s["P_A"] == len(prob.data.jA) and s["N"] == prob.data.n_atoms_total
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_descriptors(name):
+    prob = _prob(name)
+    q_o = O.descriptors(prob.data, prob.theta)
+    with H.make_gpu(prob) as nep:
+        nep.forward(want=())
+        q = nep.get_descriptors()
+    # compare in scaled units (q~ = s q is what the network sees): absolute error per component of O(1) ranges
+    err = np.max(np.abs((q - q_o) * prob.scaler))
+    assert err < 2e-5, err
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_forward_energy_force_virial(name):
+    prob = _prob(name)
+    with H.make_gpu(prob) as nep:
+        H.check_forward(nep, prob)
+        # running it twice gives the same answer up to the order of atomic additions (state is reset every call)
+        E1, F1, W1 = nep.forward()
+        E2, F2, W2 = nep.forward()
+        assert np.allclose(E1, E2, rtol=0, atol=1e-5 * prob.workload.structures.n_atoms.max())
+        assert H.relnorm(F1, F2) < 1e-5 and H.relnorm(W1, W2) < 1e-5
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_loss_and_gradient(name):
+    prob = _prob(name)
+    with H.make_gpu(prob) as nep:
+        eg, errs, g, go = H.check_grad(nep, prob, prob.workload.lambdas, per_block_tol=2e-3)
+
+
+@pytest.mark.parametrize("lam", [(1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0)])
+@pytest.mark.parametrize("name", ["tiny_T2", "cfg3"])
+def test_gradient_single_terms(name, lam):
+    prob = _prob(name)
+    with H.make_gpu(prob) as nep:
+        H.check_grad(nep, prob, lam, per_block_tol=2e-3)
+
+
+@pytest.mark.parametrize("name", ["tiny_T3_ragged", "cfg3", "cfg4"])
+def test_mini_batches(name):
+    """A batch is a list of structure ids in any order; outputs come back in batch order."""
+    prob = _prob(name)
+    S = prob.workload.structures.n_struct
+    rng = np.random.default_rng(7)
+    with H.make_gpu(prob) as nep:
+        for ids in (rng.permutation(S)[: max(1, S // 2)], [S - 1], rng.permutation(S)):
+            nep.set_batch(ids)
+            H.check_forward(nep, prob, batch=ids)
+            H.check_grad(nep, prob, (1.0, 1.0, 1.0), batch=ids)
+        nep.set_batch(None)
+        H.check_forward(nep, prob)
+
+
+def test_empty_batch_and_state_errors():
+    from paper_2606_19557_b200.binding import NepError, NEP_ESTATE, NEP_EINVAL
+    prob = _prob("tiny_T2")
+    with H.make_gpu(prob) as nep:
+        nep.set_batch([])
+        E, F, W = nep.forward()
+        assert E.shape == (0,) and F.shape == (0, 3) and W.shape == (0, 9)
+        l4 = nep.loss_grad(1.0, 1.0, 1.0)
+        assert np.all(l4 == 0.0) and np.all(nep.get_grad() == 0.0)
+        nep.set_batch(None)
+        with pytest.raises(NepError) as e:
+            nep.loss_grad(1.0, 1.0, 1.0)           # forward must come first
+        assert e.value.code == NEP_ESTATE
+        with pytest.raises(NepError) as e:
+            nep.set_batch([0, 0])
+        assert e.value.code == NEP_EINVAL
+        with pytest.raises(NepError) as e:
+            nep.set_batch([5])
+        assert e.value.code == NEP_EINVAL
+        nep.forward(want=())
+        nep.loss_grad(1.0, 1.0, 1.0)
+        nep.adam_step(1e-3)
+        with pytest.raises(NepError) as e:
+            nep.adam_step(1e-3)                    # gradient consumed
+        assert e.value.code == NEP_ESTATE
+
+
+def test_load_rejects_bad_input():
+    from paper_2606_19557_b200.binding import Nep, NepError, NEP_EINVAL
+    w = wl.tiny_workload(0)
+    st = w.structures
+    with Nep.from_model(w.model) as nep:
+        bad = st.pos.copy(); bad[0, 0] = np.nan
+        with pytest.raises(NepError) as e:
+            nep.load_structures(st.n_atoms, bad, st.box, st.type)
+        assert e.value.code == NEP_EINVAL
+        bad = st.pos.copy(); bad[0] += st.box[0].reshape(3, 3)[0] * 1.5      # outside the cell
+        with pytest.raises(NepError):
+            nep.load_structures(st.n_atoms, bad, st.box, st.type)
+        badt = st.type.copy(); badt[1] = w.model.n_species
+        with pytest.raises(NepError):
+            nep.load_structures(st.n_atoms, st.pos, st.box, badt)
+        badb = st.box.copy(); badb[0, :3] *= -1
+        with pytest.raises(NepError):
+            nep.load_structures(st.n_atoms, st.pos, badb, st.type)
+        nep.load_structures(st.n_atoms, st.pos, st.box, st.type)           # still usable afterwards
+        nep.build_neighbors()
+
+
+def test_virial_mask():
+    prob = _prob("tiny_T3_ragged")
+    hv = np.array([1, 0, 1], np.uint8)
+    prob.data.set_labels(prob.E, prob.F, prob.W, has_virial=hv)
+    try:
+        with H.make_gpu(prob) as nep:
+            nep.set_labels(prob.E, prob.F, prob.W, hv)
+            H.check_grad(nep, prob, (1.0, 2.0, 3.0), per_block_tol=2e-3)
+            nep.set_labels(prob.E, prob.F, prob.W, np.zeros(3, np.uint8))      # no virial labels at all: dV = 0
+            prob.data.set_labels(prob.E, prob.F, prob.W, has_virial=np.zeros(3, np.uint8))
+            _, _, g, go = H.check_grad(nep, prob, (1.0, 2.0, 3.0))
+    finally:
+        prob.data.set_labels(prob.E, prob.F, prob.W)
+
+
+@pytest.mark.parametrize("name", ["tiny_T2", "cfg1a", "cfg4"])
+def test_compute_scaler_matches_definition(name):
+    """Eq. 2: s = 1 / (max - min) over every loaded atom; the oracle's scaler is that definition in fp64."""
+    prob = _prob(name)
+    with H.make_gpu(prob, scaler="compute") as nep:
+        s = nep.get_scaler()
+    assert np.allclose(s, prob.scaler, rtol=2e-5), np.max(np.abs(s / prob.scaler - 1))
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_adam_same_gradient_both_sides(variant):
+    """Eqs. 9-13: three steps with the SAME gradients fed to both sides; theta within fp32 rounding."""
+    prob = _prob("cfg1a")
+    rng = np.random.default_rng(3)
+    n = prob.workload.model.n_par
+    th = prob.theta.copy(); m = np.zeros(n); v = np.zeros(n); vm = np.zeros(n); t = 0
+    with H.make_gpu(prob) as nep:
+        for _ in range(3):
+            g = (rng.normal(size=n) * 10.0 ** rng.uniform(-4, 1, size=n)).astype(np.float32)
+            t = O.adam_step(th, g.astype(np.float64), m, v, vm, t, 1e-2, 0.9, 0.999, 1e-8, variant)
+            nep.set_grad(g)
+            nep.adam_step(1e-2, 0.9, 0.999, 1e-8, variant)
+        gth = nep.get_params()
+        gm, gv, gvm, gt = nep.get_adam_state()
+    assert gt == t == 3
+    assert np.max(np.abs(gth - th)) <= 1e-6 * max(1.0, np.max(np.abs(th)))
+    assert np.allclose(gm, m, rtol=1e-5, atol=1e-12) and np.allclose(gv, v, rtol=1e-5, atol=1e-20)
+    assert np.allclose(gvm, vm, rtol=1e-5, atol=1e-20)
+
+
+def test_full_training_steps_track_the_oracle():
+    """Five full steps (forward, loss+grad, Adam) on both sides from the same start: loss trajectories agree."""
+    prob = _prob("cfg1a")
+    n = prob.workload.model.n_par
+    lam = (1.0, 1.0, 1.0)
+    th = prob.theta.copy(); m = np.zeros(n); v = np.zeros(n); vm = np.zeros(n); t = 0
+    Lo, Lg = [], []
+    with H.make_gpu(prob) as nep:
+        for _ in range(5):
+            l4o, go = O.loss_grad(prob.data, th, prob.scaler, lam)
+            t = O.adam_step(th, go, m, v, vm, t, 1e-3)
+            Lo.append(l4o[0])
+            nep.forward(want=())
+            Lg.append(nep.loss_grad(*lam)[0])
+            nep.adam_step(1e-3)
+        thg = nep.get_params()
+    assert np.allclose(Lg, Lo, rtol=1e-3), (Lg, Lo)
+    assert Lo[-1] < Lo[0]
+    assert H.relnorm(thg, th) < 1e-4
