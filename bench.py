@@ -264,7 +264,7 @@ def run_ours(args):
         Sb, Nb = nep.batch_shape()
         e_atoms += Nb
         nbs = int(np.sum((w.structures.n_atoms[ids] + 31) // 32))
-        h2d += Sb * 16 + nbs * 12
+        h2d += nbs * 16 + Sb * (16 + 4 * w.model.n_species)   # slice table, structure tables (nep_set_batch)
         d2h += 32
     b.record(); torch.cuda.synchronize()
     e2e_ms = max(a.elapsed_time(b), (time.perf_counter() - te0) * 1e3)   # host-side work (tables) is part of the call

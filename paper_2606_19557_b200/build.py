@@ -9,7 +9,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnep_b200.so")
-SOURCES = ["nep_api.cu", "nep_neighbor.cu", "nep_forward.cu", "nep_backward.cu", "nep_adam.cu"]
+SOURCES = ["nep_api.cu", "nep_neighbor.cu", "nep_ang_fwd.cu", "nep_ang_force.cu", "nep_ang_tangent.cu", "nep_ang_adjoint.cu",
+           "nep_radial.cu", "nep_ann.cu", "nep_misc.cu", "nep_adam.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 # the neighbour predicate must be bit-reproducible against the oracle: no FMA contraction in that unit
@@ -46,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(r.stderr)
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(cc, SOURCES))
     tmp = LIB + f".tmp{os.getpid()}"
     r = subprocess.run([nvcc, *ARCH, "-shared", "-o", tmp, *objs, "-lcudart"], capture_output=True, text=True)

@@ -1,0 +1,91 @@
+// nep_ang_force.cu -- S5 (angular part): the closed-form pair force of P:145 (DESIGN C8)
+//   p_ij = dE_i/dd_ij = sum_n sum_L EdS_nL [g_n'(r) b_L(r^) r^ + g_n(r) grad_d b_L(r^)],   EdS = dE_i/dS held in registers,
+// F_i += p_ij, F_j -= p_ij (one RED per component), W_s -= d_ij (x) p_ij.
+#include "nep_kernels.cuh"
+
+namespace nep {
+
+template <int NCH, int K>
+__global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
+{
+    extern __shared__ __align__(16) float smem[];
+    const ModelDev& m = a.m;
+    constexpr int CST = CoefStride<NCH, K>::value;
+    float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
+    float* cs = smem + SWEEP_SMEM_BYTES / 4;
+    const int n0 = blockIdx.y * NCH;
+    load_cA_chunk<NCH, K>(a, cs, n0);
+    __syncthreads();
+    Lane L;
+    if (!lane_init(a, L)) return;
+    const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+    float EdS[NCH][NL];
+    load_EdS<NCH>(a, L, n0, EdS);
+    float fx = 0.f, fy = 0.f, fz = 0.f, w[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) w[k] = 0.0f;
+    const float* cbase = cs + (L.ti > 0 ? L.ti : 0) * m.T * CST;
+    const float rcinv = m.rcinvA;
+    float* Fb = a.b.F;
+    const int bbase = L.bbase;
+    sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
+        const PairGeo p = pair_geo(rc4);
+        float g[NCH], dg[NCH];
+        radial_gn<NCH, K, true>(p.r, rcinv, cbase + p.tj * CST, g, dg);
+        float b[NL], A[NL];
+        const HarmZ hz = harm_z(p.z);
+        const HarmXY hxy = harm_xy(p.x, p.y);
+        harm24(hz, hxy, b);
+        float radial = 0.0f;
+#pragma unroll
+        for (int l = 0; l < NL; ++l) A[l] = 0.0f;
+#pragma unroll
+        for (int n = 0; n < NCH; ++n) {
+            float eb = 0.0f;
+#pragma unroll
+            for (int l = 0; l < NL; ++l) {
+                eb = fmaf(EdS[n][l], b[l], eb);
+                A[l] = fmaf(g[n], EdS[n][l], A[l]);
+            }
+            radial = fmaf(dg[n], eb, radial);
+        }
+        float vx, vy, vz;
+        harm24_grad_contract(hz, hxy, A, vx, vy, vz);
+        const float vr = vx * p.x + vy * p.y + vz * p.z;
+        const float px = fmaf(radial, p.x, (vx - vr * p.x) * p.rinv);
+        const float py = fmaf(radial, p.y, (vy - vr * p.y) * p.rinv);
+        const float pz = fmaf(radial, p.z, (vz - vr * p.z) * p.rinv);
+        fx += px; fy += py; fz += pz;
+        const unsigned jb = (unsigned)(bbase + p.jl);
+        float* Fj = Fb + (size_t)(jb >> 5) * (3 * WARP) + (jb & 31);
+        atomicAdd(Fj, -px); atomicAdd(Fj + WARP, -py); atomicAdd(Fj + 2 * WARP, -pz);
+        w[0] = fmaf(-p.dx, px, w[0]); w[1] = fmaf(-p.dx, py, w[1]); w[2] = fmaf(-p.dx, pz, w[2]);
+        w[3] = fmaf(-p.dy, px, w[3]); w[4] = fmaf(-p.dy, py, w[4]); w[5] = fmaf(-p.dy, pz, w[5]);
+        w[6] = fmaf(-p.dz, px, w[6]); w[7] = fmaf(-p.dz, py, w[7]); w[8] = fmaf(-p.dz, pz, w[8]);
+    });
+    if (L.ti >= 0) {
+        float* Fi = sb_ptr(Fb, L.w, 3, L.lane);
+        atomicAdd(Fi, fx); atomicAdd(Fi + WARP, fy); atomicAdd(Fi + 2 * WARP, fz);
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const float v = warp_sum(w[k]);
+        if (L.lane == 0) atomicAdd(a.b.Ws + 9 * L.sb + k, v);
+    }
+}
+
+int launch_ang_force(nep_ctx* c, const StepArgs& a)
+{
+    const ModelDev& m = c->m;
+    const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
+    const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
+    NEP_DISPATCH_NCH_K(nch, kpad, {
+        const size_t smem = SWEEP_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
+        auto kern = k_ang_force<NCH, K>;
+        if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NEP_LAUNCH(c, "k_ang_force", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+    });
+    return NEP_OK;
+}
+
+}  // namespace nep

@@ -1,0 +1,94 @@
+// nep_ang_fwd.cu -- S1 + S2 of the training step.
+// S2: angular moments S_nL = sum_j g_n(r_ij) b_L(r^_ij) (Eq. 19) and the invariants built from them: 3-body
+//     q_nl (Eq. 20), 4-/5-body (DESIGN C5).  grid = (slice pairs, channel chunks); thread = (atom, NCH channels).
+// S1: radial descriptors q_n = sum_{T'} sum_k cR[t_i][T'][n][k] B_k[T'] (Eqs. 15-16) from the one-time
+//     aggregate B, done by the threads of channel chunk 0 before their pair loop.
+#include "nep_kernels.cuh"
+
+namespace nep {
+
+template <int NCH, int K>
+__global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
+{
+    extern __shared__ __align__(16) float smem[];
+    const ModelDev& m = a.m;
+    constexpr int CST = CoefStride<NCH, K>::value;
+    float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
+    float* cs = smem + SWEEP_SMEM_BYTES / 4;
+    float* cR = cs + m.T * m.T * CST;                 // [ti][tj][n][k] as in theta (chunk 0 only)
+    const int n0 = blockIdx.y * NCH;
+    load_cA_chunk<NCH, K>(a, cs, n0);
+    if (blockIdx.y == 0)
+        for (int i = threadIdx.x; i < m.T * m.T * m.nR * m.KR; i += blockDim.x) cR[i] = a.theta[m.o_cR + i];
+    __syncthreads();
+    Lane L;
+    if (!lane_init(a, L)) return;
+    float* qp = sb_ptr(a.b.q, L.w, m.D, L.lane);
+
+    if (blockIdx.y == 0) {   // ---- S1 ----
+        // the structure accumulators that the force sweeps add into start from zero (benign duplicate stores)
+        if (L.lane < 9) a.b.Ws[9 * L.sb + L.lane] = 0.0f;
+        else if (L.lane == 9) a.b.Es[L.sb] = 0.0;
+        const float* Bp = sb_ptr(a.d.B, L.ds, m.T * m.KR, L.lane);
+        for (int n = 0; n < m.nR; ++n) {
+            float acc = 0.0f;
+            if (L.ti >= 0) {
+                const float* cc = cR + (L.ti * m.T * m.nR + n) * m.KR;
+                for (int tj = 0; tj < m.T; ++tj)
+                    for (int k = 0; k < m.KR; ++k) acc = fmaf(cc[tj * m.nR * m.KR + k], __ldg(Bp + (size_t)(tj * m.KR + k) * WARP), acc);
+            }
+            qp[(size_t)n * WARP] = acc;
+        }
+    }
+
+    // ---- S2 ----
+    const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+    float S[NCH][NL];
+#pragma unroll
+    for (int n = 0; n < NCH; ++n)
+#pragma unroll
+        for (int l = 0; l < NL; ++l) S[n][l] = 0.0f;
+    const float* cbase = cs + (L.ti > 0 ? L.ti : 0) * m.T * CST;
+    const float rcinv = m.rcinvA;
+    sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
+        const PairGeo p = pair_geo(rc4);
+        float g[NCH];
+        radial_gn<NCH, K, false>(p.r, rcinv, cbase + p.tj * CST, g, nullptr);
+        float b[NL];
+        const HarmZ hz = harm_z(p.z);
+        const HarmXY hxy = harm_xy(p.x, p.y);
+        harm24(hz, hxy, b);
+#pragma unroll
+        for (int n = 0; n < NCH; ++n)
+#pragma unroll
+            for (int l = 0; l < NL; ++l) S[n][l] = fmaf(g[n], b[l], S[n][l]);
+    });
+    float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        if (n0 + n < m.nA) {
+            float qv[6];
+            inv_values(S[n], qv);
+            store_inv(m, qp, n0 + n, qv);
+            float* sp = Sp + (size_t)(n0 + n) * NL * WARP;
+#pragma unroll
+            for (int l = 0; l < NL; ++l) sp[l * WARP] = S[n][l];
+        }
+    }
+}
+
+int launch_ang_fwd(nep_ctx* c, const StepArgs& a)
+{
+    const ModelDev& m = c->m;
+    const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
+    const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
+    NEP_DISPATCH_NCH_K(nch, kpad, {
+        const size_t smem = SWEEP_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.nR * m.KR);
+        auto kern = k_ang_fwd<NCH, K>;
+        if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NEP_LAUNCH(c, "k_ang_fwd", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+    });
+    return NEP_OK;
+}
+
+}  // namespace nep

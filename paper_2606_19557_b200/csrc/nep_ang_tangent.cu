@@ -1,0 +1,86 @@
+// nep_ang_tangent.cu -- S7 (angular part), the tangent sweep of the second-order path (DESIGN C10):
+//   Sd_nL = sum_j [g_n'(r) (r^ . d~) b_L + g_n(r) (grad_d b_L . d~)],   d~_ij = u_i - u_j - G_s^T d_ij,
+//   qd_ang = J_q(S) Sd.
+#include "nep_kernels.cuh"
+
+namespace nep {
+
+template <int NCH, int K>
+__global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
+{
+    extern __shared__ __align__(16) float smem[];
+    const ModelDev& m = a.m;
+    constexpr int CST = CoefStride<NCH, K>::value;
+    float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
+    float* cs = smem + SWEEP_SMEM_BYTES / 4;
+    const int n0 = blockIdx.y * NCH;
+    load_cA_chunk<NCH, K>(a, cs, n0);
+    __syncthreads();
+    Lane L;
+    if (!lane_init(a, L)) return;
+    const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+    float G[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) G[k] = __ldg(a.b.G + 9 * L.sb + k);
+    const float* ui = sb_ptr(a.b.u, L.w, 3, L.lane);
+    const float uix = ui[0], uiy = ui[WARP], uiz = ui[2 * WARP];
+    float Sd[NCH][NL];
+#pragma unroll
+    for (int n = 0; n < NCH; ++n)
+#pragma unroll
+        for (int l = 0; l < NL; ++l) Sd[n][l] = 0.0f;
+    const float* cbase = cs + (L.ti > 0 ? L.ti : 0) * m.T * CST;
+    const float rcinv = m.rcinvA;
+    const float* ub = a.b.u;
+    const int bbase = L.bbase;
+    sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
+        const PairGeo p = pair_geo(rc4);
+        const Tangent T = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
+        float g[NCH], dg[NCH];
+        radial_gn<NCH, K, true>(p.r, rcinv, cbase + p.tj * CST, g, dg);
+        float b[NL], bd[NL];
+        const HarmZ hz = harm_z(p.z);
+        const HarmXY hxy = harm_xy(p.x, p.y);
+        harm24(hz, hxy, b);
+        harm24_tangent(hz, hxy, T.rx, T.ry, T.rz, bd);
+#pragma unroll
+        for (int n = 0; n < NCH; ++n) {
+            const float c1 = dg[n] * T.t;
+#pragma unroll
+            for (int l = 0; l < NL; ++l) Sd[n][l] = fmaf(c1, b[l], fmaf(g[n], bd[l], Sd[n][l]));
+        }
+    });
+    const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
+    float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
+    float* qdp = sb_ptr(a.b.qd, L.w, m.D, L.lane);
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        if (n0 + n < m.nA) {
+            float S[NL], qd[6];
+            const size_t o = (size_t)(n0 + n) * NL * WARP;
+#pragma unroll
+            for (int l = 0; l < NL; ++l) {
+                S[l] = Sp[o + l * WARP];
+                Sdp[o + l * WARP] = Sd[n][l];
+            }
+            inv_tangent(S, Sd[n], qd);
+            store_inv(m, qdp, n0 + n, qd);
+        }
+    }
+}
+
+int launch_ang_tangent(nep_ctx* c, const StepArgs& a)
+{
+    const ModelDev& m = c->m;
+    const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
+    const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
+    NEP_DISPATCH_NCH_K(nch, kpad, {
+        const size_t smem = SWEEP_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
+        auto kern = k_ang_tangent<NCH, K>;
+        if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NEP_LAUNCH(c, "k_ang_tangent", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+    });
+    return NEP_OK;
+}
+
+}  // namespace nep

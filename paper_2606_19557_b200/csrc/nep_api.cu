@@ -76,7 +76,7 @@ static int upload(nep_ctx* c, T*& dptr, const T* h, size_t count)
 
 extern "C" {
 
-const char* nep_version(void) { return "nep_b200 0.1 (sm_100a, fp32 step, fp64 neighbour predicate)"; }
+const char* nep_version(void) { return "nep_b200 0.2 (sm_100a, fp32 step, fp64 neighbour predicate)"; }
 
 const char* nep_last_error(const nep_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
@@ -139,6 +139,7 @@ int nep_destroy(nep_ctx* c)
     cudaStreamSynchronize(c->stream);
     std::vector<void*> a = c->allocs;
     for (void* p : a) dev_free(c, p);
+    if (c->h_stage) cudaFreeHost(c->h_stage);
     for (auto& r : c->prof.pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto e : c->prof.pool) cudaEventDestroy(e);
     delete c;
@@ -151,7 +152,7 @@ int64_t nep_num_params(const nep_ctx* c) { return c ? c->m.npar : NEP_EINVAL; }
 static void free_dataset(nep_ctx* c)
 {
     DataDev& d = c->d;
-    const void* ptrs[] = { d.pos, d.box, d.type, d.atom_off, d.pbase, d.type_p, d.slice_struct, d.Elab, d.Flab, d.Wlab, d.hasv,
+    const void* ptrs[] = { d.pos, d.box, d.type, d.atom_off, d.pbase, d.type_p, d.rank_p, d.slice_struct, d.Elab, d.Flab, d.Wlab, d.hasv,
                            d.offR, d.jR, d.shR, d.offA, d.jA, d.shA, d.cntR, d.recoffR, d.recR, d.cntA, d.recoffA, d.recA, d.B };
     for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
     memset(&d, 0, sizeof d);
@@ -169,7 +170,10 @@ static int upload_labels(nep_ctx* c, const double* E, const double* F, const dou
     std::vector<float> Fp((size_t)3 * c->NP, 0.0f), Wf((size_t)9 * c->S);
     for (int s = 0; s < c->S; ++s)
         for (int i = 0; i < c->h_nat[s]; ++i)
-            for (int k = 0; k < 3; ++k) Fp[(size_t)k * c->NP + c->h_pbase[s] + i] = (float)F[3 * (c->h_aoff[s] + i) + k];
+            for (int k = 0; k < 3; ++k) {   // slice-blocked [slice][3][32]
+                const int64_t p = c->h_pbase[s] + i;
+                Fp[(size_t)((p / WARP) * 3 + k) * WARP + p % WARP] = (float)F[3 * (c->h_aoff[s] + i) + k];
+            }
     for (size_t i = 0; i < Wf.size(); ++i) Wf[i] = (float)W[i];
     c->h_hasv.assign(c->S, 1);
     if (hv) for (int s = 0; s < c->S; ++s) c->h_hasv[s] = hv[s] ? 1 : 0;
@@ -224,24 +228,31 @@ int nep_load_structures(nep_ctx* c, int S, const int* n_atoms, const double* pos
     free_dataset(c);
     c->S = S; c->N = N; c->NP = NP; c->nslices = (int)(NP / WARP);
     c->h_nat.assign(n_atoms, n_atoms + S); c->h_aoff = aoff; c->h_pbase = pbase; c->h_box.assign(box, box + 9 * (size_t)S);
-    std::vector<int> type_p((size_t)NP, -1), slice_struct((size_t)c->nslices, 0);
+    std::vector<int> type_p((size_t)NP, -1), rank_p((size_t)NP, 0), slice_struct((size_t)c->nslices, 0);
+    c->h_tcount.assign((size_t)S * c->m.T, 0);
     for (int s = 0; s < S; ++s) {
-        for (int i = 0; i < n_atoms[s]; ++i) type_p[pbase[s] + i] = type[aoff[s] + i];
+        int* tc = &c->h_tcount[(size_t)s * c->m.T];
+        for (int i = 0; i < n_atoms[s]; ++i) {
+            const int t = type[aoff[s] + i];
+            type_p[pbase[s] + i] = t;
+            rank_p[pbase[s] + i] = tc[t]++;
+        }
         for (int64_t sl = pbase[s] / WARP; sl < pbase[s + 1] / WARP; ++sl) slice_struct[sl] = s;
     }
     DataDev& d = c->d;
     d.S = S; d.N = N; d.NP = NP; d.nslices = c->nslices;
     int rc;
-    double *dpos, *dbox; int *dtype, *dtp, *dss; int64_t *dao, *dpb;
+    double *dpos, *dbox; int *dtype, *dtp, *drk, *dss; int64_t *dao, *dpb;
     if ((rc = upload<double>(c, dpos, pos, 3 * (size_t)N))) return rc;
     if ((rc = upload<double>(c, dbox, box, 9 * (size_t)S))) return rc;
     if ((rc = upload<int>(c, dtype, type, (size_t)N))) return rc;
     if ((rc = upload<int>(c, dtp, type_p.data(), type_p.size()))) return rc;
+    if ((rc = upload<int>(c, drk, rank_p.data(), rank_p.size()))) return rc;
     if ((rc = upload<int>(c, dss, slice_struct.data(), slice_struct.size()))) return rc;
     if ((rc = upload<int64_t>(c, dao, aoff.data(), aoff.size()))) return rc;
     if ((rc = upload<int64_t>(c, dpb, pbase.data(), pbase.size()))) return rc;
     NEP_CUDA(c, cudaStreamSynchronize(c->stream));
-    d.pos = dpos; d.box = dbox; d.type = dtype; d.type_p = dtp; d.slice_struct = dss; d.atom_off = dao; d.pbase = dpb;
+    d.pos = dpos; d.box = dbox; d.type = dtype; d.type_p = dtp; d.rank_p = drk; d.slice_struct = dss; d.atom_off = dao; d.pbase = dpb;
     c->have_data = true;
     if (lab) return upload_labels(c, E, F, W, has_virial);
     c->h_hasv.assign(S, 1);
@@ -387,38 +398,51 @@ int nep_compute_scaler(nep_ctx* c)
     return NEP_OK;
 }
 
-static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs)
+static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64_t tiles_m)
 {
     BatchDev& b = c->b;
     const ModelDev& m = c->m;
     if (NBP > c->cap_NBP) {
-        void* olds[] = { b.q, b.Fp, b.h, b.S, b.Sd, b.qd, b.Qb, b.arow, b.Bd, b.F, b.u, b.Ei };
+        void* olds[] = { b.q, b.Fp, b.S, b.Sd, b.qd, b.Qb, b.arow, b.Bd, b.F, b.u, b.Ei };
         for (void* p : olds) dev_free(c, p);
         size_t n = (size_t)NBP;
-        ALLOC(c, b.q, float, n * m.D);   ALLOC(c, b.Fp, float, n * m.D);  ALLOC(c, b.h, float, n * m.H);
+        ALLOC(c, b.q, float, n * m.D);   ALLOC(c, b.Fp, float, n * m.D);
         ALLOC(c, b.S, float, n * m.nA * 24); ALLOC(c, b.Sd, float, n * m.nA * 24);
         ALLOC(c, b.qd, float, n * m.D);  ALLOC(c, b.Qb, float, n * m.D);
         ALLOC(c, b.arow, float, n * m.T * m.KRP); ALLOC(c, b.Bd, float, n * m.T * m.KR);
         ALLOC(c, b.F, float, n * 3);     ALLOC(c, b.u, float, n * 3);     ALLOC(c, b.Ei, float, n);
         c->cap_NBP = NBP;
     }
+    if (tiles_m > c->cap_tiles_m) {
+        dev_free(c, b.alist); dev_free(c, b.hbuf);
+        ALLOC(c, b.alist, int, tiles_m);
+        ALLOC(c, b.hbuf, float, (size_t)tiles_m * m.HP);
+        c->cap_tiles_m = tiles_m;
+    }
     if (Sb > c->cap_Sb) {
-        void* olds[] = { b.Es, b.Ws, b.eps, b.G, (void*)b.bsid, (void*)b.bnat, (void*)b.bfoff };
+        void* olds[] = { b.Es, b.Ws, b.eps, b.G };
         for (void* p : olds) dev_free(c, p);
         ALLOC(c, b.Es, double, Sb); ALLOC(c, b.Ws, float, 9 * (size_t)Sb); ALLOC(c, b.eps, float, Sb); ALLOC(c, b.G, float, 9 * (size_t)Sb);
-        int* p1; int* p2; int64_t* p3;
-        ALLOC(c, p1, int, Sb); ALLOC(c, p2, int, Sb); ALLOC(c, p3, int64_t, Sb);
-        b.bsid = p1; b.bnat = p2; b.bfoff = p3;
         c->cap_Sb = Sb;
     }
-    if (nbs > c->cap_nbs) {
-        dev_free(c, (void*)b.bslice); dev_free(c, (void*)b.bsb); dev_free(c, (void*)b.bbase);
-        int *p1, *p2, *p3;
-        ALLOC(c, p1, int, nbs); ALLOC(c, p2, int, nbs); ALLOC(c, p3, int, nbs);
-        b.bslice = p1; b.bsb = p2; b.bbase = p3;
-        c->cap_nbs = nbs;
+    if (!b.lacc) {   // loss accumulators and the block ticket: zero once, the loss kernel re-arms them itself
+        ALLOC(c, b.lacc, double, 8); ALLOC(c, b.counter, unsigned, 4);
+        NEP_CUDA(c, cudaMemsetAsync(b.lacc, 0, 64, c->stream));
+        NEP_CUDA(c, cudaMemsetAsync(b.counter, 0, 16, c->stream));
     }
-    if (!b.lacc) ALLOC(c, b.lacc, double, 8);
+    // per-batch tables: one pinned host block, one device block, one copy per nep_set_batch
+    const size_t need = 16 * (size_t)nbs + 8 * (size_t)Sb + 4 * (size_t)Sb * (2 + m.T) + 64;
+    if (need > c->d_stage_bytes) {
+        NEP_CUDA(c, cudaStreamSynchronize(c->stream));   // no copy out of the old pinned block is pending
+        dev_free(c, c->d_stage);
+        if (c->h_stage) cudaFreeHost(c->h_stage);
+        c->h_stage = nullptr; c->d_stage = nullptr; c->d_stage_bytes = 0;
+        const size_t cap = need + need / 2;
+        NEP_CUDA(c, cudaMallocHost(&c->h_stage, cap));
+        c->d_stage = dev_alloc(c, cap);
+        if (!c->d_stage) return NEP_ENOMEM;
+        c->d_stage_bytes = c->h_stage_bytes = cap;
+    }
     return NEP_OK;
 }
 
@@ -427,43 +451,64 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
     CHECK_CTX(c);
     if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_set_batch before nep_build_neighbors");
     if (ids && n < 0) return fail(c, NEP_EINVAL, "negative batch size");
-    int Sb = ids ? n : c->S;
-    std::vector<int> bsid(Sb), bnat(Sb), bslice, bsb, bbase;
-    std::vector<int64_t> bfoff(Sb);
+    const int Sb = ids ? n : c->S;
+    const int T = c->m.T;
     std::vector<unsigned char> seen(ids ? c->S : 0, 0);
-    int64_t Nb = 0, nbp = 0, PRb = 0, PAb = 0;
-    int Sv = 0;
+    int64_t nbs64 = 0;
     for (int k = 0; k < Sb; ++k) {
-        int s = ids ? ids[k] : k;
+        const int s = ids ? ids[k] : k;
         if (s < 0 || s >= c->S) return fail(c, NEP_EINVAL, "structure id out of range");
         if (ids) { if (seen[s]) return fail(c, NEP_EINVAL, "duplicate structure id in batch"); seen[s] = 1; }
+        nbs64 += (c->h_pbase[s + 1] - c->h_pbase[s]) / WARP;
+    }
+    if (nbs64 * WARP > INT32_MAX / 2) return fail(c, NEP_ECAPACITY, "batch too large");
+    const int nbs = (int)nbs64;
+    // network tiles: atoms sorted by species, every species padded to whole tiles
+    const int TM = ann_tile_m(c);
+    std::vector<int64_t> tot(T, 0);
+    for (int k = 0; k < Sb; ++k) {
+        const int s = ids ? ids[k] : k;
+        for (int t = 0; t < T; ++t) tot[t] += c->h_tcount[(size_t)s * T + t];
+    }
+    BatchDev& b = c->b;
+    int ntiles = 0;
+    for (int t = 0; t < T; ++t) { b.tile_start[t] = ntiles; ntiles += (int)((tot[t] + TM - 1) / TM); }
+    for (int t = T; t <= MAX_T; ++t) b.tile_start[t] = ntiles;
+    int rc = ensure_batch_capacity(c, std::max<int64_t>(nbs64 * WARP, WARP), std::max(Sb, 1), std::max(nbs, 1), std::max<int64_t>((int64_t)ntiles * TM, TM));
+    if (rc) return rc;
+    // tables, packed: binfo [nbs] int4 | bfoff [Sb] int64 | bsid [Sb] | bnat [Sb] | bsoff [Sb][T]
+    char* h = (char*)c->h_stage;
+    int4* binfo = (int4*)h;
+    int64_t* bfoff = (int64_t*)(h + 16 * (size_t)nbs);
+    int* bsid = (int*)(bfoff + Sb);
+    int* bnat = bsid + Sb;
+    int* bsoff = bnat + Sb;
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));   // the previous copy out of the pinned block has finished
+    int64_t Nb = 0, nbp = 0, PRb = 0, PAb = 0;
+    int Sv = 0, w = 0;
+    std::vector<int> run(T, 0);
+    for (int k = 0; k < Sb; ++k) {
+        const int s = ids ? ids[k] : k;
         bsid[k] = s; bnat[k] = c->h_nat[s]; bfoff[k] = Nb;
+        for (int t = 0; t < T; ++t) { bsoff[(size_t)k * T + t] = run[t]; run[t] += c->h_tcount[(size_t)s * T + t]; }
         Nb += c->h_nat[s];
         Sv += c->h_hasv.empty() ? 1 : c->h_hasv[s];
         PRb += c->h_pairsR_struct[s]; PAb += c->h_pairsA_struct[s];
-        for (int64_t sl = c->h_pbase[s] / WARP; sl < c->h_pbase[s + 1] / WARP; ++sl) {
-            bslice.push_back((int)sl); bsb.push_back(k); bbase.push_back((int)nbp);
-        }
+        for (int64_t sl = c->h_pbase[s] / WARP; sl < c->h_pbase[s + 1] / WARP; ++sl) binfo[w++] = make_int4((int)sl, k, (int)nbp, 0);
         nbp += c->h_pbase[s + 1] - c->h_pbase[s];
-        if (nbp > INT32_MAX / 2) return fail(c, NEP_ECAPACITY, "batch too large");
     }
-    int nbs = (int)bslice.size();
-    int rc = ensure_batch_capacity(c, std::max<int64_t>(nbp, WARP), std::max(Sb, 1), std::max(nbs, 1));
-    if (rc) return rc;
-    BatchDev& b = c->b;
-    b.Sb = Sb; b.Sv = Sv; b.Nb = Nb; b.nbs = nbs; b.NBP = nbp;
-    if (Sb) {
-        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bsid, bsid.data(), 4 * (size_t)Sb, cudaMemcpyHostToDevice, c->stream));
-        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bnat, bnat.data(), 4 * (size_t)Sb, cudaMemcpyHostToDevice, c->stream));
-        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bfoff, bfoff.data(), 8 * (size_t)Sb, cudaMemcpyHostToDevice, c->stream));
-        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bslice, bslice.data(), 4 * (size_t)nbs, cudaMemcpyHostToDevice, c->stream));
-        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bsb, bsb.data(), 4 * (size_t)nbs, cudaMemcpyHostToDevice, c->stream));
-        NEP_CUDA(c, cudaMemcpyAsync((void*)b.bbase, bbase.data(), 4 * (size_t)nbs, cudaMemcpyHostToDevice, c->stream));
-        NEP_CUDA(c, cudaStreamSynchronize(c->stream));   // host vectors die at return
-    }
-    c->h_bsid = bsid; c->h_bfoff = bfoff; c->PRb = PRb; c->PAb = PAb;
+    b.Sb = Sb; b.Sv = Sv; b.Nb = Nb; b.nbs = nbs; b.NBP = nbp; b.tile_m = TM; b.ntiles = ntiles;
+    const size_t bytes = 16 * (size_t)nbs + 8 * (size_t)Sb + 4 * (size_t)Sb * (2 + T);
+    char* d = (char*)c->d_stage;
+    b.binfo = (const int4*)d;
+    b.bfoff = (const int64_t*)(d + 16 * (size_t)nbs);
+    b.bsid = (const int*)(b.bfoff + Sb);
+    b.bnat = b.bsid + Sb;
+    b.bsoff = b.bnat + Sb;
+    if (bytes) NEP_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, bytes, cudaMemcpyHostToDevice, c->stream));
+    c->h_bsid.assign(bsid, bsid + Sb); c->h_bfoff.assign(bfoff, bfoff + Sb); c->PRb = PRb; c->PAb = PAb;
     c->forward_valid = c->grad_valid = false;
-    return NEP_OK;
+    return launch_build_alist(c);
 }
 
 static int copy_out(nep_ctx* c, void* dst, const float* src, size_t count, int on_host)

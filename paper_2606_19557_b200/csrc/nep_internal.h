@@ -1,4 +1,9 @@
 // nep_internal.h -- context, device views and launcher declarations shared by the .cu files of libnep_b200.
+//
+// Data layout.  Atoms of a structure are cut into SLICES of 32 (one warp = one slice, one
+// lane = one atom, the last slice of a structure padded).  Every per-atom array the pair sweeps touch is
+// "slice-blocked": element (slice w, row r, lane l) lives at ((w * ROWS) + r) * 32 + l, so a warp reads or writes
+// 128 contiguous bytes per row and the row offset is an immediate in the instruction.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -17,7 +22,7 @@ constexpr int MAX_NCH = 5;   // angular channels held in registers by one thread
 
 // Everything a kernel needs to know about the model (passed by value).
 struct ModelDev {
-    int T, nR, nA, KR, KA, KRP, H, HP, D, DP, nang, has4, has5;   // HP, DP: H, D padded to multiples of 8
+    int T, nR, nA, KR, KA, KRP, H, HP, D, DP, nang, has4, has5;   // HP, DP: H, D padded to multiples of 8; KRP: KR to 4
     float rcR, rcA, rcinvR, rcinvA;
     // offsets into theta
     int per_type;          // (D + 2) * H
@@ -29,7 +34,7 @@ struct ModelDev {
 struct DataDev {
     int S;                 // structures
     int64_t N;             // atoms
-    int64_t NP;            // padded atoms: every structure padded to a multiple of 32 (one warp = one slice)
+    int64_t NP;            // padded atoms: every structure padded to a multiple of 32
     int nslices;           // NP / 32
     const double* pos;     // [N][3]
     const double* box;     // [S][9]
@@ -37,10 +42,11 @@ struct DataDev {
     const int64_t* atom_off;   // [S+1]
     const int64_t* pbase;      // [S+1] padded offset of each structure
     const int* type_p;     // [NP], -1 = padding
+    const int* rank_p;     // [NP] rank of the atom among the atoms of its own type in its structure
     const int* slice_struct;   // [nslices]
     // labels
     const double* Elab;    // [S]
-    const float* Flab;     // [3][NP]
+    const float* Flab;     // [nslices][3][32]
     const float* Wlab;     // [S][9]
     const unsigned char* hasv; // [S]
     // canonical neighbour lists (CSR over the N atoms)
@@ -49,40 +55,46 @@ struct DataDev {
     // sliced pair cache: record (slice, slot s, lane) at rec[recoff[slice] + s*32 + lane]
     const int* cntR; const int64_t* recoffR; const float4* recR;
     const int* cntA; const int64_t* recoffA; const float4* recA;
-    const float* B;        // [T*KR][NP] radial aggregate  B_k[T'] = sum_{j in N_R(i), t_j = T'} f_k(r_ij)
+    const float* B;        // [nslices][T*KR][32] radial aggregate  B_k[T'] = sum_{j in N_R(i), t_j = T'} f_k(r_ij)
 };
 
-// Current mini-batch: a list of slices, all per-step temporaries are indexed by batch-padded atom ib = w*32 + lane.
+// Current mini-batch: a list of slices; per-step temporaries are slice-blocked over the batch slices.
 struct BatchDev {
     int Sb;                // structures in the batch
     int Sv;                // ... of which have virial labels
     int64_t Nb;            // atoms in the batch
     int nbs;               // slices in the batch
     int64_t NBP;           // nbs * 32
-    const int* bslice;     // [nbs] data-set slice id
-    const int* bsb;        // [nbs] batch structure index of the slice
-    const int* bbase;      // [nbs] batch-padded index of the first atom of the slice's structure
+    const int4* binfo;     // [nbs] {data-set slice, batch structure index, batch-padded index of the structure's first atom, 0}
     const int* bsid;       // [Sb]  data-set structure id
     const int* bnat;       // [Sb]  atoms of the structure
     const int64_t* bfoff;  // [Sb]  first atom in batch order (unpadded), for outputs
+    const int* bsoff;      // [Sb][T] atoms of type t in the earlier structures of the batch
+    // network tiles: atoms of the batch sorted by type, each type padded to a multiple of the tile size
+    int tile_m;            // atoms per tile (128 or 64)
+    int ntiles;
+    int tile_start[MAX_T + 1];   // first tile of each type
+    int* alist;            // [ntiles * tile_m] batch-padded atom index, -1 = padding
     // temporaries
-    float* q;      // [D][NBP]   unscaled descriptors
-    float* Fp;     // [D][NBP]   dE_i/dq
-    float* h;      // [H][NBP]   tanh
-    float* S;      // [nA*24][NBP] normalised angular moments
-    float* Sd;     // [nA*24][NBP] their tangent
-    float* qd;     // [D][NBP]   tangent of q (angular part written by the tangent sweep, radial by the network kernel)
-    float* Qb;     // [D][NBP]   adjoint of q
-    float* arow;   // [NBP][T][KRP]  a_k[T'] = sum_n Fp_n cR[t_i][T'][n][k]
-    float* Bd;     // [T*KR][NBP] tangent of B
-    float* F;      // [3][NBP]
-    float* u;      // [3][NBP]   dL/dF
-    float* Ei;     // [NBP]
+    float* q;      // [nbs][D][32]   unscaled descriptors
+    float* Fp;     // [nbs][D][32]   dE_i/dq
+    float* qd;     // [nbs][D][32]   tangent of q (angular rows; radial rows are formed inside the network kernel)
+    float* Qb;     // [nbs][D][32]   adjoint of q
+    float* S;      // [nbs][nA*24][32] normalised angular moments
+    float* Sd;     // [nbs][nA*24][32] their tangent
+    float* hbuf;   // [ntiles][HP][tile_m] tanh outputs, tile order
+    float* arow;   // [NBP][T*KRP]   a_k[T'] = sum_n Fp_n cR[t_i][T'][n][k]
+    float* Bd;     // [nbs][T*KR][32] tangent of B
+    float* F;      // [nbs][3][32]
+    float* u;      // [nbs][3][32]   dL/dF
+    float* Ei;     // [nbs][32]
+    // per structure
     double* Es;    // [Sb]
     float* Ws;     // [Sb][9]
     float* eps;    // [Sb]       dL/dE_s
     float* G;      // [Sb][9]    dL/dW_s
-    double* lacc;  // [4] sums: (dE)^2, |dF|^2, (dW)^2, spare ; loss4 at [4..7]
+    double* lacc;  // [8] sums: (dE)^2, |dF|^2, (dW)^2, spare ; loss4 at [4..7]
+    unsigned* counter;   // [4] block ticket of the loss kernel
 };
 
 struct Profiler {
@@ -108,6 +120,7 @@ struct nep_ctx {
     // host copies of the data set
     int S = 0; int64_t N = 0, NP = 0; int nslices = 0;
     std::vector<int> h_nat; std::vector<int64_t> h_aoff, h_pbase; std::vector<unsigned char> h_hasv;
+    std::vector<int> h_tcount;   // [S][T] atoms of each type
     std::vector<double> h_box;
     bool have_data = false, have_labels = false, have_nbrs = false, have_params = false, have_scaler = false;
     bool forward_valid = false, grad_valid = false;
@@ -115,10 +128,12 @@ struct nep_ctx {
 
     nep::DataDev d{};
     nep::BatchDev b{};
-    int64_t cap_NBP = 0; int cap_Sb = 0; int cap_nbs = 0;
+    int64_t cap_NBP = 0; int cap_Sb = 0; int cap_nbs = 0; int64_t cap_tiles_m = 0;
     std::vector<int> h_bsid; std::vector<int64_t> h_bfoff;
     int64_t PRb = 0, PAb = 0;
     std::vector<int64_t> h_pairsR_struct, h_pairsA_struct;   // pairs per structure (for sizes / flop models)
+    // pinned staging for the per-batch tables (one async copy per nep_set_batch)
+    void* h_stage = nullptr; size_t h_stage_bytes = 0; void* d_stage = nullptr; size_t d_stage_bytes = 0;
 
     float *theta = nullptr, *g = nullptr, *am = nullptr, *av = nullptr, *avmax = nullptr, *scaler = nullptr;
     int64_t t_adam = 0;
@@ -146,11 +161,13 @@ void prof_end(nep_ctx* c);
 
 // ---- launchers (each returns NEP_OK or an error code with c->err set) ----
 int build_neighbors_dev(nep_ctx* c);                           // nep_neighbor.cu : S0a + S0b
-int launch_forward(nep_ctx* c, bool descriptors_only);         // nep_forward.cu  : S1-S5
-int launch_loss_grad(nep_ctx* c);                              // nep_backward.cu : S6-S9
+int launch_forward(nep_ctx* c, bool descriptors_only);         // nep_step.cu     : S1-S5
+int launch_loss_grad(nep_ctx* c);                              // nep_step.cu     : S6-S9
 int launch_adam(nep_ctx* c, double lr, double b1, double b2, double eps, int variant);  // nep_adam.cu : S10
-int launch_scaler_minmax(nep_ctx* c, float* d_s);              // nep_forward.cu  : S0c (after a descriptors-only pass over all)
-int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW);  // nep_forward.cu: batch-padded -> batch order
+int launch_scaler_minmax(nep_ctx* c, float* d_s);              // nep_misc.cu     : S0c (after a descriptors-only pass over all)
+int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW);  // nep_misc.cu: slice-blocked -> batch order
 int launch_gather_q(nep_ctx* c, float* dq);                    // [N_b][D]
+int launch_build_alist(nep_ctx* c);                            // nep_misc.cu     : type-sorted atom list of the batch
+int ann_tile_m(const nep_ctx* c);                              // nep_ann.cu      : atoms per network tile for this model
 
 }  // namespace nep

@@ -1,9 +1,11 @@
-// nep_kernels.cuh -- helpers shared by the step kernels (forward, backward).
+// nep_kernels.cuh -- helpers shared by the step kernels.
 //
 // Execution model of every pair sweep: ONE THREAD PER ATOM, one warp per 32-atom slice of one structure.
 // Pair records of a slice are stored slot-major ([slot][lane], 16 B each), so the 32 lanes of a warp read
-// 512 contiguous bytes per slot; each lane's records are sorted by neighbour type.  Per-atom tensors
-// (angular moments and their adjoints, up to 5 channels x 24 harmonics) live in registers.
+// 512 contiguous bytes per slot; each lane's records are sorted by neighbour type.  The record of slot s+1 is
+// fetched before slot s is processed.  Per-atom tensors (angular moments and their adjoints, up to 5 channels x
+// 24 harmonics) live in registers; all sizes that shape a loop (channels per thread, basis functions) are
+// compile-time constants so that no register array is indexed dynamically.
 #pragma once
 #include "nep_internal.h"
 #include "nep_math.cuh"
@@ -17,29 +19,32 @@ struct StepArgs {
     const float* theta;
     const float* scaler;
     float* g;
-    int nchunks, nAP;   // angular channel chunks (blockIdx.y) and padded channel count nchunks * NCH
+    int nchunks;   // angular channel chunks (blockIdx.y)
 };
 
+constexpr int PAIR_TB = 64;   // threads per block of the pair sweeps (2 slices)
+
 struct Lane {
-    int w, lane, ti, sb, bbase;
-    int64_t ib, ip;
-    int ds;
+    int w, lane, ds, sb, bbase, ti;
+    unsigned ib;   // batch-padded atom index w*32 + lane
 };
 
 // false if the warp is beyond the batch (whole warp returns together)
 __device__ __forceinline__ bool lane_init(const StepArgs& a, Lane& L)
 {
-    L.w = (int)((blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5);
+    L.w = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     L.lane = threadIdx.x & 31;
     if (L.w >= a.b.nbs) return false;
-    L.ds = a.b.bslice[L.w];
-    L.sb = a.b.bsb[L.w];
-    L.bbase = a.b.bbase[L.w];
-    L.ib = (int64_t)L.w * WARP + L.lane;
-    L.ip = (int64_t)L.ds * WARP + L.lane;
-    L.ti = a.d.type_p[L.ip];
+    const int4 bi = __ldg(a.b.binfo + L.w);
+    L.ds = bi.x; L.sb = bi.y; L.bbase = bi.z;
+    L.ib = (unsigned)L.w * WARP + L.lane;
+    L.ti = __ldg(a.d.type_p + (size_t)L.ds * WARP + L.lane);
     return true;
 }
+
+// slice-blocked addressing: row 0 of (slice, lane) in an array with ROWS rows per slice
+__device__ __forceinline__ float* sb_ptr(float* base, int slice, int rows, int lane) { return base + ((size_t)slice * rows) * WARP + lane; }
+__device__ __forceinline__ const float* sb_ptr(const float* base, int slice, int rows, int lane) { return base + ((size_t)slice * rows) * WARP + lane; }
 
 __device__ __forceinline__ float warp_sum(float v)
 {
@@ -71,31 +76,138 @@ __device__ __forceinline__ PairGeo pair_geo(const float4& rec)
     return p;
 }
 
-// g_n(r) = sum_k c[k][n] f_k(r) (and g_n'), n = 0..NCH-1, coefficients at cs[k * nAP + n]  (Eq. 16)
-template <int NCH, bool DERIV>
-__device__ __forceinline__ void radial_gn(float r, float rcinv, int K, const float* __restrict__ cs, int nAP, float* g, float* dg)
+// Streams the pair records of one lane: body(record) for slots 0..cnt-1; all lanes of the warp walk `width` slots.
+// Records are staged through shared memory with cp.async (LDGSTS), SWEEP_STAGES slots ahead, so that the HBM/L2
+// latency of slot s+1, s+2 is covered by the arithmetic of slot s.  Each lane reads back only what it copied
+// itself, so cp.async.wait_group is the only synchronisation needed.
+constexpr int SWEEP_STAGES = 2;
+constexpr int SWEEP_SMEM_BYTES = PAIR_TB * 16 * SWEEP_STAGES;   // per block, at the start of dynamic shared memory
+
+__device__ __forceinline__ void cp_async16(float4* smem_dst, const float4* gsrc)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(s), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+
+// stage: this thread's first staging cell, cells of successive stages are PAIR_TB apart.
+// pre(active, record) runs converged on every lane of the warp for every slot (votes are allowed in it);
+// body(record) runs on the lanes that still have a record in this slot.
+template <class Pre, class Body>
+__device__ __forceinline__ void sweep_pairs(const float4* __restrict__ rec, int width, int cnt, float4* stage, Pre&& pre, Body&& body)
+{
+#pragma unroll
+    for (int st = 0; st < SWEEP_STAGES; ++st) {
+        if (st < width) cp_async16(stage + st * PAIR_TB, rec + (size_t)st * WARP);
+        cp_async_commit();
+    }
+    for (int s = 0; s < width; ++s) {
+        cp_async_wait<SWEEP_STAGES - 1>();
+        float4* cell = stage + (s % SWEEP_STAGES) * PAIR_TB;
+        const float4 cur = *cell;
+        if (s + SWEEP_STAGES < width) cp_async16(cell, rec + (size_t)(s + SWEEP_STAGES) * WARP);
+        cp_async_commit();
+        pre(s < cnt, cur);
+        if (s < cnt) body(cur);
+    }
+    cp_async_wait<0>();
+}
+template <class Body>
+__device__ __forceinline__ void sweep_pairs(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body&& body)
+{
+    sweep_pairs(rec, width, cnt, stage, [](bool, const float4&) {}, body);
+}
+
+struct SweepA { const float4* rec; int width, cnt; };
+__device__ __forceinline__ SweepA sweep_init(const int64_t* __restrict__ recoff, const float4* __restrict__ recs,
+                                             const int* __restrict__ cntp, const Lane& L)
+{
+    SweepA s;
+    const int64_t base = __ldg(recoff + L.ds);
+    s.width = (int)((__ldg(recoff + L.ds + 1) - base) >> 5);
+    s.rec = recs + base + L.lane;
+    s.cnt = (L.ti >= 0) ? __ldg(cntp + (size_t)L.ds * WARP + L.lane) : 0;
+    return s;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Angular coefficients of one channel chunk in shared memory: cs[pt * CSTRIDE + k * NCHP + n], n < NCHP (zero
+// padded), NCHP = 4 (NCH <= 4) or 8; CSTRIDE = K * NCHP rounded up to 4 (mod 8) so that the 128-bit loads of
+// lanes with different pair types fall into different bank groups.
+// ------------------------------------------------------------------------------------------------
+template <int NCH> struct ChunkPad { static constexpr int value = NCH <= 4 ? 4 : 8; };
+template <int NCH, int K> struct CoefStride {
+    static constexpr int raw = K * ChunkPad<NCH>::value;
+    static constexpr int value = raw + ((12 - raw % 8) % 8);   // == 4 (mod 8)
+};
+
+template <int NCH, int K>
+__device__ __forceinline__ void load_cA_chunk(const StepArgs& a, float* cs, int n0)
+{
+    const ModelDev& m = a.m;
+    constexpr int NCHP = ChunkPad<NCH>::value, CST = CoefStride<NCH, K>::value;
+    const int tot = m.T * m.T * CST;
+    for (int i = threadIdx.x; i < tot; i += blockDim.x) {
+        const int pt = i / CST, rem = i - pt * CST, k = rem / NCHP, n = rem - k * NCHP;
+        float v = 0.0f;
+        if (k < m.KA && n < NCH && n0 + n < m.nA) v = a.theta[m.o_cA + (pt * m.nA + n0 + n) * m.KA + k];
+        cs[i] = v;
+    }
+}
+template <int NCH, int K>
+inline size_t cA_chunk_bytes(const ModelDev& m) { return 4 * (size_t)(m.T * m.T * CoefStride<NCH, K>::value); }
+
+// coefficients of basis function k for the NCH channels of the chunk
+template <int NCH>
+__device__ __forceinline__ void coef_k(const float* __restrict__ cp, int k, float* c)
+{
+    constexpr int NCHP = ChunkPad<NCH>::value;
+    const float4 v = *reinterpret_cast<const float4*>(cp + k * NCHP);
+    c[0] = v.x;
+    if (NCH > 1) c[1] = v.y;
+    if (NCH > 2) c[2] = v.z;
+    if (NCH > 3) c[3] = v.w;
+    if (NCH > 4) c[4] = cp[k * NCHP + 4];
+}
+
+// g_n(r) = sum_k c_nk f_k(r) (and g_n') for the chunk's channels  (Eq. 16)
+template <int NCH, int K, bool DERIV>
+__device__ __forceinline__ void radial_gn(float r, float rcinv, const float* __restrict__ cp, float* g, float* dg)
 {
 #pragma unroll
     for (int n = 0; n < NCH; ++n) { g[n] = 0.0f; if (DERIV) dg[n] = 0.0f; }
-    cheb_foreach<17>(r, rcinv, K, [&](int k, float fk, float dfk) {
+    cheb_basis<K, DERIV>(r, rcinv, [&](int k, float fk, float dfk) {
+        float c[NCH];
+        coef_k<NCH>(cp, k, c);
 #pragma unroll
         for (int n = 0; n < NCH; ++n) {
-            const float c = cs[k * nAP + n];
-            g[n] = fmaf(c, fk, g[n]);
-            if (DERIV) dg[n] = fmaf(c, dfk, dg[n]);
+            g[n] = fmaf(c[n], fk, g[n]);
+            if (DERIV) dg[n] = fmaf(c[n], dfk, dg[n]);
         }
     });
 }
 
-// copies the angular coefficients of theta into shared memory as [pair type][k][n padded to nAP]
-__device__ __forceinline__ void load_cA_smem(const StepArgs& a, float* cs)
+// descriptor rows of the angular invariants of channel n: slots 0..3 -> l = 1..4, slot 4 -> 4-body, slot 5 -> 5-body
+__device__ __forceinline__ int ang_row(const ModelDev& m, int slot, int n)
 {
-    const ModelDev& m = a.m;
-    const int tot = m.T * m.T * m.KA * a.nAP;
-    for (int i = threadIdx.x; i < tot; i += blockDim.x) {
-        const int n = i % a.nAP, k = (i / a.nAP) % m.KA, pt = i / (a.nAP * m.KA);
-        cs[i] = (n < m.nA) ? a.theta[m.o_cA + (pt * m.nA + n) * m.KA + k] : 0.0f;
-    }
+    const int a = slot < 4 ? slot : (slot == 4 ? 4 : 4 + m.has4);
+    return m.nR + a * m.nA + n;
+}
+// c[slot] = arr[row(slot, n)] for the invariants present, 0 otherwise  (arr: slice-blocked [D] rows, pointer at row 0)
+__device__ __forceinline__ void load_inv_coef(const ModelDev& m, const float* __restrict__ arr, int n, float* c)
+{
+#pragma unroll
+    for (int s = 0; s < 4; ++s) c[s] = arr[(size_t)ang_row(m, s, n) * WARP];
+    c[4] = m.has4 ? arr[(size_t)ang_row(m, 4, n) * WARP] : 0.0f;
+    c[5] = m.has5 ? arr[(size_t)ang_row(m, 5, n) * WARP] : 0.0f;
+}
+__device__ __forceinline__ void store_inv(const ModelDev& m, float* __restrict__ arr, int n, const float* q)
+{
+#pragma unroll
+    for (int s = 0; s < 4; ++s) arr[(size_t)ang_row(m, s, n) * WARP] = q[s];
+    if (m.has4) arr[(size_t)ang_row(m, 4, n) * WARP] = q[4];
+    if (m.has5) arr[(size_t)ang_row(m, 5, n) * WARP] = q[5];
 }
 
 // EdS_nL = dE_i/dS_nL = sum_a Fp[q index (a, n)] dq_a/dS_nL for the NCH channels of this thread (DESIGN C8)
@@ -103,20 +215,39 @@ template <int NCH>
 __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n0, float (*EdS)[NL])
 {
     const ModelDev& m = a.m;
+    const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
+    const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
 #pragma unroll
     for (int n = 0; n < NCH; ++n) {
         if (n0 + n < m.nA && L.ti >= 0) {
             float S[NL], coef[6];
+            const float* sp = Sp + (size_t)(n0 + n) * NL * WARP;
 #pragma unroll
-            for (int l = 0; l < NL; ++l) S[l] = a.b.S[(int64_t)((n0 + n) * NL + l) * a.b.NBP + L.ib];
-#pragma unroll
-            for (int aa = 0; aa < 6; ++aa) coef[aa] = (aa < m.nang) ? a.b.Fp[(int64_t)(m.nR + aa * m.nA + n0 + n) * a.b.NBP + L.ib] : 0.0f;
-            inv_adjoint(S, m.has4, m.has5, coef, EdS[n]);
+            for (int l = 0; l < NL; ++l) S[l] = sp[l * WARP];
+            load_inv_coef(m, Fpp, n0 + n, coef);
+            inv_adjoint(S, coef, EdS[n]);
         } else {
 #pragma unroll
             for (int l = 0; l < NL; ++l) EdS[n][l] = 0.0f;
         }
     }
+}
+
+// d~ = u_i - u_j - G^T d ;  returns t = r^ . d~ and the tangent rho = (d~ - t r^) / r of r^
+struct Tangent { float t, rx, ry, rz; };
+__device__ __forceinline__ Tangent pair_tangent(const float* __restrict__ ub, int bbase, const PairGeo& p, float uix, float uiy, float uiz,
+                                                const float* G)
+{
+    const unsigned jb = (unsigned)(bbase + p.jl);
+    const float* uj = ub + (size_t)(jb >> 5) * (3 * WARP) + (jb & 31);
+    const float ujx = __ldg(uj), ujy = __ldg(uj + WARP), ujz = __ldg(uj + 2 * WARP);
+    const float tx = uix - ujx - (G[0] * p.dx + G[3] * p.dy + G[6] * p.dz);
+    const float ty = uiy - ujy - (G[1] * p.dx + G[4] * p.dy + G[7] * p.dz);
+    const float tz = uiz - ujz - (G[2] * p.dx + G[5] * p.dy + G[8] * p.dz);
+    Tangent T;
+    T.t = tx * p.x + ty * p.y + tz * p.z;
+    T.rx = (tx - T.t * p.x) * p.rinv; T.ry = (ty - T.t * p.y) * p.rinv; T.rz = (tz - T.t * p.z) * p.rinv;
+    return T;
 }
 
 #define NEP_LAUNCH(c, name, kernel, grid, block, smem, ...)                        \
@@ -127,19 +258,45 @@ __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n
         NEP_CUDA((c), cudaGetLastError());                                         \
     } while (0)
 
-inline StepArgs make_args(nep_ctx* c, int NCH)
+// channels per thread for the angular sweeps: 3, 4 or 5 (fewer channels run as 3 with zero coefficients)
+inline int pick_nch(int nA)
+{
+    const int chunks = (nA + MAX_NCH - 1) / MAX_NCH;
+    const int nch = (nA + chunks - 1) / chunks;
+    return nch < 3 ? 3 : nch;
+}
+inline int pick_kpad(int K) { return K <= 9 ? 9 : (K <= 13 ? 13 : 17); }
+
+inline StepArgs make_args(nep_ctx* c)
 {
     StepArgs a;
     a.m = c->m; a.d = c->d; a.b = c->b; a.theta = c->theta; a.scaler = c->scaler; a.g = c->g;
-    a.nchunks = (c->m.nA + NCH - 1) / NCH; a.nAP = a.nchunks * NCH;
+    const int nch = pick_nch(c->m.nA);
+    a.nchunks = (c->m.nA + nch - 1) / nch;
     return a;
 }
-// channels per thread for the angular sweeps: ceil(nA / ceil(nA / 5)), at least 2
-inline int pick_nch(int nA)
-{
-    int chunks = (nA + MAX_NCH - 1) / MAX_NCH;
-    int nch = (nA + chunks - 1) / chunks;
-    return nch < 2 ? 2 : nch;
-}
+
+// instantiates `__VA_ARGS__` with constexpr int NCH, K for the model's channel count and basis size
+#define NEP_DISPATCH_NCH_K(nch, kpad, ...)                                              \
+    do {                                                                                \
+        if ((nch) == 3) { constexpr int NCH = 3; NEP_DISPATCH_K_(kpad, __VA_ARGS__) }   \
+        else if ((nch) == 4) { constexpr int NCH = 4; NEP_DISPATCH_K_(kpad, __VA_ARGS__) } \
+        else { constexpr int NCH = 5; NEP_DISPATCH_K_(kpad, __VA_ARGS__) }              \
+    } while (0)
+#define NEP_DISPATCH_K_(kpad, ...)                          \
+    if ((kpad) == 9) { constexpr int K = 9; __VA_ARGS__; }  \
+    else if ((kpad) == 13) { constexpr int K = 13; __VA_ARGS__; } \
+    else { constexpr int K = 17; __VA_ARGS__; }
+
+// launchers of the individual sweeps (one .cu file each, so that they compile in parallel)
+int launch_ang_fwd(nep_ctx* c, const StepArgs& a);
+int launch_ang_force(nep_ctx* c, const StepArgs& a);
+int launch_ang_tangent(nep_ctx* c, const StepArgs& a);
+int launch_ang_adjoint(nep_ctx* c, const StepArgs& a);
+int launch_rad_force(nep_ctx* c, const StepArgs& a);
+int launch_rad_tangent(nep_ctx* c, const StepArgs& a);
+int launch_ann_fwd(nep_ctx* c, const StepArgs& a);
+int launch_ann_bwd(nep_ctx* c, const StepArgs& a);
+int launch_loss(nep_ctx* c, const StepArgs& a);
 
 }  // namespace nep

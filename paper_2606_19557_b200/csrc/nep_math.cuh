@@ -25,32 +25,62 @@ constexpr float C5 = 7.0f / 15.0f;               // q5 = kappa5 |s|^4 = (7/15) q
 constexpr float PI_F = 3.14159265358979323846f;
 
 // ------------------------------------------------------------------------------------------------
-// Chebyshev x cosine-cutoff basis.  body(k, f_k, df_k/dr) is called for k = 0..K-1 (K <= KMAX).
+// cos(pi u), sin(pi u) for u in [0, 1]  (the only range Eq. 18 needs: 0 < r < rc).
+// v = u - 1/2 in [-1/2, 1/2]:  cos(pi u) = -sin(pi v), sin(pi u) = cos(pi v); Taylor polynomials in x = pi v,
+// |x| <= pi/2, truncated after x^13 / x^14 (first neglected terms 5.7e-8 x and 6.4e-9): ~1 ulp of the results that
+// Eqs. 17-18 use them for, at 15 FMA-pipe operations (sincospif costs ~25 with its range reduction and selects).
 // ------------------------------------------------------------------------------------------------
-template <int KMAX, class Body>
-__device__ __forceinline__ void cheb_foreach(float r, float rcinv, int K, Body&& body)
+__device__ __forceinline__ void sincospi_unit(float u, float& sn, float& cs)
+{
+    const float x = PI_F * (u - 0.5f);
+    const float x2 = x * x;
+    float ps = -1.0f / 6227020800.0f;                       // -1/13!
+    ps = fmaf(ps, x2, 1.0f / 39916800.0f);                  //  1/11!
+    ps = fmaf(ps, x2, -1.0f / 362880.0f);
+    ps = fmaf(ps, x2, 1.0f / 5040.0f);
+    ps = fmaf(ps, x2, -1.0f / 120.0f);
+    ps = fmaf(ps, x2, 1.0f / 6.0f);
+    ps = ps * x2;                                           // (x - sin x) / x
+    float pc = 1.0f / 479001600.0f;                         //  1/12!
+    pc = fmaf(pc, x2, -1.0f / 3628800.0f);
+    pc = fmaf(pc, x2, 1.0f / 40320.0f);
+    pc = fmaf(pc, x2, -1.0f / 720.0f);
+    pc = fmaf(pc, x2, 1.0f / 24.0f);
+    pc = fmaf(pc, x2, -0.5f);
+    cs = fmaf(ps, x, -x);                                   // cos(pi u) = -sin x
+    sn = fmaf(pc, x2, 1.0f);                                // sin(pi u) =  cos x
+}
+
+// ------------------------------------------------------------------------------------------------
+// Chebyshev x cosine-cutoff basis (Eqs. 17-18).  body(k, f_k, df_k/dr) is called for k = 0..K-1, K a compile-time
+// constant (models with fewer functions run the next larger instantiation with zero-padded coefficients).
+// Without DERIV the derivative argument is 0 and its arithmetic is not generated.
+// ------------------------------------------------------------------------------------------------
+template <int K, bool DERIV, class Body>
+__device__ __forceinline__ void cheb_basis(float r, float rcinv, Body&& body)
 {
     const float u = r * rcinv;
     float sn, cs;
-    sincospif(u, &sn, &cs);
-    const float hfc = 0.25f * (cs + 1.0f);               // 1/2 f_c
-    const float hdfc = -0.25f * PI_F * rcinv * sn;       // 1/2 f_c'
+    sincospi_unit(u, sn, cs);
+    const float hfc = fmaf(0.25f, cs, 0.25f);              // 1/2 f_c
     const float um1 = u - 1.0f;
-    const float x = 2.0f * um1 * um1 - 1.0f;
-    const float hdxfc = 4.0f * um1 * rcinv * hfc;        // 1/2 x' f_c
+    const float x = fmaf(2.0f * um1, um1, -1.0f);
     const float x2 = 2.0f * x;
+    float hdfc = 0.0f, hdxfc = 0.0f;
+    if (DERIV) {
+        hdfc = (-0.25f * PI_F) * rcinv * sn;               // 1/2 f_c'
+        hdxfc = 4.0f * um1 * rcinv * hfc;                  // 1/2 x' f_c
+    }
     float T2 = 1.0f, T1 = x, dT2 = 0.0f, dT1 = 1.0f;
     body(0, 2.0f * hfc, 2.0f * hdfc);
-    if (K > 1) body(1, (x + 1.0f) * hfc, fmaf(x + 1.0f, hdfc, hdxfc));
+    if (K > 1) body(1, fmaf(x, hfc, hfc), DERIV ? fmaf(x, hdfc, hdfc + hdxfc) : 0.0f);
 #pragma unroll
-    for (int k = 2; k < KMAX; ++k) {
-        if (k < K) {
-            const float T = fmaf(x2, T1, -T2);
-            const float dT = fmaf(x2, dT1, fmaf(2.0f, T1, -dT2));
-            T2 = T1; T1 = T; dT2 = dT1; dT1 = dT;
-            const float tp = T + 1.0f;
-            body(k, tp * hfc, fmaf(dT, hdxfc, tp * hdfc));
-        }
+    for (int k = 2; k < K; ++k) {
+        const float T = fmaf(x2, T1, -T2);
+        float dT = 0.0f;
+        if (DERIV) dT = fmaf(x2, dT1, fmaf(2.0f, T1, -dT2));
+        T2 = T1; T1 = T; dT2 = dT1; dT1 = dT;
+        body(k, fmaf(T, hfc, hfc), DERIV ? fmaf(dT, hdxfc, fmaf(T, hdfc, hdfc)) : 0.0f);
     }
 }
 
@@ -219,76 +249,59 @@ __device__ __forceinline__ float ldot(const float* S, const float* V, int l)
     return s;
 }
 
-// q[0..5]: values of the invariants
-__device__ __forceinline__ void inv_values(const float* S, bool has4, bool has5, float* q)
+// Invariants of one channel.  q[0..3]: l = 1..4 (Eq. 20); q[4]: 4-body; q[5]: 5-body (always at these fixed slots;
+// the caller maps them to descriptor rows).  coefficient arrays c[6] use the same slots (0 where a term is absent).
+__device__ __forceinline__ void inv_values(const float* S, float* q)
 {
     q[0] = lsum(S, 1); q[1] = lsum(S, 2); q[2] = lsum(S, 3); q[3] = lsum(S, 4);
-    int a = 4;
-    if (has4) {
-        const Sym6 T = tensor_from_l2(S);
-        Sym6 T2 = anticomm(T, T);
-        q[a++] = 0.5f * KAPPA4 * sym_dot(T2, T);
-    }
-    if (has5) q[a++] = C5 * q[0] * q[0];
+    const Sym6 T = tensor_from_l2(S);
+    const Sym6 T2 = anticomm(T, T);
+    q[4] = 0.5f * KAPPA4 * sym_dot(T2, T);
+    q[5] = C5 * q[0] * q[0];
 }
-// out[L] = sum_a coef[a] dq_a/dS_L
-__device__ __forceinline__ void inv_adjoint(const float* S, bool has4, bool has5, const float* coef, float* out)
+// out[L] = sum_a c[a] dq_a/dS_L
+__device__ __forceinline__ void inv_adjoint(const float* S, const float* c, float* out)
 {
-    float c1 = 2.0f * coef[0];
-    int a = 4;
-    if (has4) ++a;
-    if (has5) c1 = fmaf(4.0f * C5 * coef[a], lsum(S, 1), c1);   // d/dS (7/15) q1^2 = (28/15) q1 S
+    const float c1 = fmaf(4.0f * C5 * c[5], lsum(S, 1), 2.0f * c[0]);   // d/dS (7/15) q1^2 = (28/15) q1 S
 #pragma unroll
     for (int L = 0; L < 3; ++L) out[L] = c1 * S[L];
 #pragma unroll
-    for (int L = 3; L < 8; ++L) out[L] = 2.0f * coef[1] * S[L];
+    for (int L = 3; L < 8; ++L) out[L] = 2.0f * c[1] * S[L];
 #pragma unroll
-    for (int L = 8; L < 15; ++L) out[L] = 2.0f * coef[2] * S[L];
+    for (int L = 8; L < 15; ++L) out[L] = 2.0f * c[2] * S[L];
 #pragma unroll
-    for (int L = 15; L < 24; ++L) out[L] = 2.0f * coef[3] * S[L];
-    if (has4) {
-        const Sym6 T = tensor_from_l2(S);
-        Sym6 P = anticomm(T, T);   // 2 T^2 ; dq4/dT = 3 kappa4 T^2
-        l2_from_tensor_adjoint(P, 1.5f * KAPPA4 * coef[4], out);
-    }
+    for (int L = 15; L < 24; ++L) out[L] = 2.0f * c[3] * S[L];
+    const Sym6 T = tensor_from_l2(S);
+    const Sym6 P = anticomm(T, T);   // 2 T^2 ; dq4/dT = 3 kappa4 T^2
+    l2_from_tensor_adjoint(P, 1.5f * KAPPA4 * c[4], out);
 }
 // qd[a] = sum_L dq_a/dS_L * V_L
-__device__ __forceinline__ void inv_tangent(const float* S, const float* V, bool has4, bool has5, float* qd)
+__device__ __forceinline__ void inv_tangent(const float* S, const float* V, float* qd)
 {
     qd[0] = 2.0f * ldot(S, V, 1); qd[1] = 2.0f * ldot(S, V, 2); qd[2] = 2.0f * ldot(S, V, 3); qd[3] = 2.0f * ldot(S, V, 4);
-    int a = 4;
-    if (has4) {
-        const Sym6 T = tensor_from_l2(S), Td = tensor_from_l2(V);
-        Sym6 T2 = anticomm(T, T);
-        qd[a++] = 1.5f * KAPPA4 * sym_dot(T2, Td);
-    }
-    if (has5) qd[a++] = 2.0f * C5 * lsum(S, 1) * qd[0];
+    const Sym6 T = tensor_from_l2(S), Td = tensor_from_l2(V);
+    const Sym6 T2 = anticomm(T, T);
+    qd[4] = 1.5f * KAPPA4 * sym_dot(T2, Td);
+    qd[5] = 2.0f * C5 * lsum(S, 1) * qd[0];
 }
-// out[L] += sum_a coef[a] sum_L' (d2 q_a / dS_L dS_L') V_L'
-__device__ __forceinline__ void inv_hessian_action(const float* S, const float* V, bool has4, bool has5, const float* coef, float* out)
+// out[L] += sum_a c[a] sum_L' (d2 q_a / dS_L dS_L') V_L'
+__device__ __forceinline__ void inv_hessian_action(const float* S, const float* V, const float* c, float* out)
 {
-    int a = 4;
-    if (has4) ++a;
-    float c1 = 2.0f * coef[0], c1s = 0.0f;
-    if (has5) {
-        // d/dS_L [(28/15) q1 S_L] along V: (28/15) (q1d S_L + q1 V_L), q1d = 2 S.V
-        const float q1 = lsum(S, 1), q1d = 2.0f * ldot(S, V, 1);
-        c1 = fmaf(4.0f * C5 * coef[a], q1, c1);
-        c1s = 4.0f * C5 * coef[a] * q1d;
-    }
+    // d/dS_L [(28/15) q1 S_L] along V: (28/15) (q1d S_L + q1 V_L), q1d = 2 S.V
+    const float q1 = lsum(S, 1), q1d = 2.0f * ldot(S, V, 1);
+    const float c1 = fmaf(4.0f * C5 * c[5], q1, 2.0f * c[0]);
+    const float c1s = 4.0f * C5 * c[5] * q1d;
 #pragma unroll
     for (int L = 0; L < 3; ++L) out[L] += fmaf(c1, V[L], c1s * S[L]);
 #pragma unroll
-    for (int L = 3; L < 8; ++L) out[L] = fmaf(2.0f * coef[1], V[L], out[L]);
+    for (int L = 3; L < 8; ++L) out[L] = fmaf(2.0f * c[1], V[L], out[L]);
 #pragma unroll
-    for (int L = 8; L < 15; ++L) out[L] = fmaf(2.0f * coef[2], V[L], out[L]);
+    for (int L = 8; L < 15; ++L) out[L] = fmaf(2.0f * c[2], V[L], out[L]);
 #pragma unroll
-    for (int L = 15; L < 24; ++L) out[L] = fmaf(2.0f * coef[3], V[L], out[L]);
-    if (has4) {
-        const Sym6 T = tensor_from_l2(S), Td = tensor_from_l2(V);
-        Sym6 Pd = anticomm(T, Td);   // T Td + Td T ; d(3 k4 T^2) = 3 k4 (T Td + Td T)
-        l2_from_tensor_adjoint(Pd, 3.0f * KAPPA4 * coef[4], out);
-    }
+    for (int L = 15; L < 24; ++L) out[L] = fmaf(2.0f * c[3], V[L], out[L]);
+    const Sym6 T = tensor_from_l2(S), Td = tensor_from_l2(V);
+    const Sym6 Pd = anticomm(T, Td);   // T Td + Td T ; d(3 k4 T^2) = 3 k4 (T Td + Td T)
+    l2_from_tensor_adjoint(Pd, 3.0f * KAPPA4 * c[4], out);
 }
 
 }  // namespace nep

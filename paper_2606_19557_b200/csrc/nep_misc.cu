@@ -1,0 +1,229 @@
+// nep_misc.cu -- S6 (loss and its seeds, Eqs. 4-7) in one kernel, the type-sorted atom list of the batch,
+// the descriptor scaler (S0c, Eq. 2) and the re-ordering of outputs from the slice-blocked layout to batch order.
+#include <algorithm>
+
+#include "nep_kernels.cuh"
+
+namespace nep {
+
+// ------------------------------------------------------------------------------------------------
+// S6.  thread = batch-padded atom: u_i = dL/dF_i = 2 lF (F_i - F_i^lab) / (3 N_b), sum |dF|^2          (Eq. 6)
+//      thread < S_b also = structure: eps_s = dL/dE_s, G_s = dL/dW_s, sums of (dE/N)^2, (dW/N)^2       (Eqs. 5, 7)
+//      every thread clears its share of g (the sweeps that follow accumulate into it);
+//      the last block to finish forms L (Eq. 4) and g_b1 = -sum_s eps_s N_s, and re-arms the accumulators.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF, float lamV, double dlamE, double dlamF, double dlamV)
+{
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nthreads = gridDim.x * blockDim.x;
+    for (int i = gid; i < a.m.npar; i += nthreads) a.g[i] = 0.0f;
+    double sF = 0.0, sE = 0.0, sW = 0.0, sB = 0.0;
+    if (gid < a.b.NBP) {
+        const int w = gid >> 5, lane = gid & 31;
+        const int4 bi = __ldg(a.b.binfo + w);
+        const bool valid = __ldg(a.d.type_p + (size_t)bi.x * WARP + lane) >= 0;
+        const float c = 2.0f * lamF / (3.0f * (float)a.b.Nb);
+        const float* Fp = sb_ptr(a.b.F, w, 3, lane);
+        const float* Fl = sb_ptr(a.d.Flab, bi.x, 3, lane);
+        float* up = sb_ptr(a.b.u, w, 3, lane);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const float dF = valid ? Fp[k * WARP] - __ldg(Fl + k * WARP) : 0.0f;
+            sF += (double)dF * (double)dF;
+            up[k * WARP] = c * dF;
+        }
+    }
+    if (gid < a.b.Sb) {
+        const int sb = gid;
+        const int sid = a.b.bsid[sb];
+        const double n = (double)a.b.bnat[sb];
+        const double dE = a.b.Es[sb] - a.d.Elab[sid];
+        sE = (dE / n) * (dE / n);                                                   // Eq. 5
+        const float eps = (float)(2.0 * dlamE * dE / ((double)a.b.Sb * n * n));
+        a.b.eps[sb] = eps;
+        sB = (double)eps * n;
+        const bool hv = a.d.hasv[sid] != 0;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+            const double t = hv ? (double)a.b.Ws[9 * sb + k] - (double)a.d.Wlab[9 * (size_t)sid + k] : 0.0;
+            sW += (t / n) * (t / n);                                                // Eq. 7
+            a.b.G[9 * sb + k] = (hv && a.b.Sv > 0) ? (float)(2.0 * dlamV * t / (9.0 * a.b.Sv * n * n)) : 0.0f;
+        }
+    }
+    // block reduction -> one atomic per block and quantity
+    __shared__ double red[4][8];
+    __shared__ bool last;
+    sF = warp_sum(sF); sE = warp_sum(sE); sW = warp_sum(sW); sB = warp_sum(sB);
+    const int wid = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) { red[0][wid] = sE; red[1][wid] = sF; red[2][wid] = sW; red[3][wid] = sB; }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += red[threadIdx.x][w];
+        if (s != 0.0) atomicAdd(a.b.lacc + threadIdx.x, s);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) last = (atomicAdd(a.b.counter, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        volatile double* l = a.b.lacc;
+        const double dE = a.b.Sb ? l[0] / a.b.Sb : 0.0, dF = a.b.Nb ? l[1] / (3.0 * a.b.Nb) : 0.0, dV = a.b.Sv ? l[2] / (9.0 * a.b.Sv) : 0.0;
+        const double sb1 = l[3];
+        l[4] = dlamE * dE + dlamF * dF + dlamV * dV; l[5] = dE; l[6] = dF; l[7] = dV;   // Eq. 4
+        a.g[a.m.o_b1] = (float)(-sb1);                                                   // g_b1 = -sum_i eps_s(i)
+        l[0] = 0.0; l[1] = 0.0; l[2] = 0.0; l[3] = 0.0;
+        *a.b.counter = 0u;
+    }
+}
+
+int launch_loss(nep_ctx* c, const StepArgs& a)
+{
+    const int64_t n = std::max<int64_t>(c->b.NBP, 1);
+    NEP_LAUNCH(c, "k_loss", k_loss, (unsigned)((n + 255) / 256), 256, 0, a, (float)c->lamE, (float)c->lamF, (float)c->lamV,
+               c->lamE, c->lamF, c->lamV);
+    return NEP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Type-sorted atom list of the batch (tiles of the network kernels).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_build_alist(StepArgs a)
+{
+    const int ib = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ib >= a.b.NBP) return;
+    const int w = ib >> 5, lane = ib & 31;
+    const int4 bi = __ldg(a.b.binfo + w);
+    const size_t ip = (size_t)bi.x * WARP + lane;
+    const int t = a.d.type_p[ip];
+    if (t < 0) return;
+    const int pos = a.b.tile_start[t] * a.b.tile_m + a.b.bsoff[bi.y * a.m.T + t] + a.d.rank_p[ip];
+    a.b.alist[pos] = ib;
+}
+
+int launch_build_alist(nep_ctx* c)
+{
+    if (c->b.ntiles == 0) return NEP_OK;
+    NEP_CUDA(c, cudaMemsetAsync(c->b.alist, 0xFF, 4 * (size_t)c->b.ntiles * c->b.tile_m, c->stream));
+    StepArgs a = make_args(c);
+    NEP_LAUNCH(c, "k_build_alist", k_build_alist, (unsigned)((c->b.NBP + 255) / 256), 256, 0, a);
+    return NEP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// outputs in batch order, descriptors, scaler
+// ------------------------------------------------------------------------------------------------
+__global__ void k_gather_outputs(StepArgs a, float* E, float* F, float* W)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < a.b.Sb) {
+        if (E) E[i] = (float)a.b.Es[i];
+        if (W) for (int k = 0; k < 9; ++k) W[9 * i + k] = a.b.Ws[9 * i + k];
+    }
+    if (F && i < a.b.NBP) {
+        const int w = (int)(i >> 5), lane = (int)(i & 31);
+        const int4 bi = a.b.binfo[w];
+        if (a.d.type_p[(size_t)bi.x * WARP + lane] >= 0) {
+            const int64_t o = a.b.bfoff[bi.y] + (i - bi.z);
+            const float* Fp = sb_ptr(a.b.F, w, 3, lane);
+            F[3 * o] = Fp[0]; F[3 * o + 1] = Fp[WARP]; F[3 * o + 2] = Fp[2 * WARP];
+        }
+    }
+}
+__global__ void k_gather_q(StepArgs a, float* q)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= a.b.NBP) return;
+    const int w = (int)(i >> 5), lane = (int)(i & 31);
+    const int4 bi = a.b.binfo[w];
+    if (a.d.type_p[(size_t)bi.x * WARP + lane] < 0) return;
+    const int64_t o = a.b.bfoff[bi.y] + (i - bi.z);
+    const float* qp = sb_ptr(a.b.q, w, a.m.D, lane);
+    for (int v = 0; v < a.m.D; ++v) q[o * a.m.D + v] = qp[(size_t)v * WARP];
+}
+// S0c (Eq. 2): one block per descriptor component: s = 1 / (max - min), degenerate range -> 1 (DESIGN G10)
+__global__ void __launch_bounds__(256) k_scaler_minmax(StepArgs a, float* s)
+{
+    const int v = blockIdx.x;
+    float lo = INFINITY, hi = -INFINITY, am = 0.0f;
+    for (int64_t i = threadIdx.x; i < a.b.NBP; i += blockDim.x) {
+        const int w = (int)(i >> 5), lane = (int)(i & 31);
+        const int ds = a.b.binfo[w].x;
+        if (a.d.type_p[(size_t)ds * WARP + lane] >= 0) {
+            const float x = sb_ptr(a.b.q, w, a.m.D, lane)[(size_t)v * WARP];
+            lo = fminf(lo, x); hi = fmaxf(hi, x); am = fmaxf(am, fabsf(x));
+        }
+    }
+    __shared__ float slo[256], shi[256], sam[256];
+    slo[threadIdx.x] = lo; shi[threadIdx.x] = hi; sam[threadIdx.x] = am;
+    __syncthreads();
+    for (int o = 128; o; o >>= 1) {
+        if (threadIdx.x < o) {
+            slo[threadIdx.x] = fminf(slo[threadIdx.x], slo[threadIdx.x + o]);
+            shi[threadIdx.x] = fmaxf(shi[threadIdx.x], shi[threadIdx.x + o]);
+            sam[threadIdx.x] = fmaxf(sam[threadIdx.x], sam[threadIdx.x + o]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const float range = shi[0] - slo[0];
+        s[v] = (a.b.Nb > 0 && range > 1e-12f * fmaxf(1.0f, sam[0])) ? 1.0f / range : 1.0f;
+    }
+}
+
+int launch_scaler_minmax(nep_ctx* c, float* d_s)
+{
+    StepArgs a = make_args(c);
+    NEP_CUDA(c, cudaMemsetAsync(d_s, 0, 4 * (size_t)c->m.DP, c->stream));
+    NEP_LAUNCH(c, "k_scaler_minmax", k_scaler_minmax, c->m.D, 256, 0, a, d_s);
+    return NEP_OK;
+}
+
+int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW)
+{
+    StepArgs a = make_args(c);
+    const int64_t n = std::max<int64_t>(c->b.NBP, c->b.Sb);
+    if (n == 0) return NEP_OK;
+    NEP_LAUNCH(c, "k_gather_outputs", k_gather_outputs, (unsigned)((n + 255) / 256), 256, 0, a, dE, dF, dW);
+    return NEP_OK;
+}
+
+int launch_gather_q(nep_ctx* c, float* dq)
+{
+    StepArgs a = make_args(c);
+    if (c->b.NBP == 0) return NEP_OK;
+    NEP_LAUNCH(c, "k_gather_q", k_gather_q, (unsigned)((c->b.NBP + 255) / 256), 256, 0, a, dq);
+    return NEP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// the step: order of the sweeps
+// ------------------------------------------------------------------------------------------------
+int launch_forward(nep_ctx* c, bool descriptors_only)
+{
+    if (c->b.nbs == 0) return NEP_OK;
+    const StepArgs a = make_args(c);
+    int rc;
+    if ((rc = launch_ang_fwd(c, a))) return rc;        // S1 + S2 (also clears E_s, W_s of the batch)
+    if (descriptors_only) return NEP_OK;
+    if ((rc = launch_ann_fwd(c, a))) return rc;        // S3
+    if ((rc = launch_rad_force(c, a))) return rc;      // S5 radial + S4
+    if ((rc = launch_ang_force(c, a))) return rc;      // S5 angular
+    return NEP_OK;
+}
+
+int launch_loss_grad(nep_ctx* c)
+{
+    const StepArgs a = make_args(c);
+    int rc;
+    if ((rc = launch_loss(c, a))) return rc;           // S6 (clears g)
+    if (c->b.nbs == 0) return NEP_OK;
+    if ((rc = launch_rad_tangent(c, a))) return rc;    // S7 radial
+    if ((rc = launch_ang_tangent(c, a))) return rc;    // S7 angular
+    if ((rc = launch_ann_bwd(c, a))) return rc;        // S8
+    if ((rc = launch_ang_adjoint(c, a))) return rc;    // S9
+    return NEP_OK;
+}
+
+}  // namespace nep

@@ -217,7 +217,8 @@ __device__ void basis_f64(double r, double rc, int K, double* f)
 }
 
 // One thread per padded atom: writes the atom's pair records sorted by neighbour type (stable in canonical order),
-// record = (dx, dy, dz, bits) with bits = j_local | t_j << 24.  RADIAL also accumulates B_k[T'] in fp64.
+// record = (dx, dy, dz, bits) with bits = j_local | t_j << 24.  RADIAL also accumulates B_k[T'] in fp64
+// (slice-blocked: B[slice][T' * KR + k][lane]).
 template <bool RADIAL>
 __global__ void k_cache_fill(int nslices, ModelDev m, const double* __restrict__ pos, const double* __restrict__ box,
                              const int* __restrict__ type, const int64_t* __restrict__ pbase, const int64_t* __restrict__ atom_off,
@@ -229,7 +230,7 @@ __global__ void k_cache_fill(int nslices, ModelDev m, const double* __restrict__
     if (sl >= nslices) return;
     int64_t ip = (int64_t)sl * WARP + lane;
     if (type_p[ip] < 0) {
-        if (RADIAL) for (int k = 0; k < m.T * m.KR; ++k) B[(int64_t)k * NP + ip] = 0.0f;
+        if (RADIAL) for (int k = 0; k < m.T * m.KR; ++k) B[((int64_t)sl * m.T * m.KR + k) * WARP + lane] = 0.0f;
         return;
     }
     int s = slice_struct[sl];
@@ -258,7 +259,7 @@ __global__ void k_cache_fill(int nslices, ModelDev m, const double* __restrict__
                 for (int k = 0; k < m.KR; ++k) acc[k] += f[k];
             }
         }
-        if (RADIAL) for (int k = 0; k < m.KR; ++k) B[(int64_t)(t * m.KR + k) * NP + ip] = (float)acc[k];
+        if (RADIAL) for (int k = 0; k < m.KR; ++k) B[((int64_t)sl * m.T * m.KR + t * m.KR + k) * WARP + lane] = (float)acc[k];
     }
 }
 

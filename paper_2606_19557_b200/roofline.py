@@ -34,9 +34,9 @@ def kernel_models(model, sizes: dict) -> dict:
     KRP = (KR + 3) // 4 * 4
     f4 = 4
     m = {}
-    m["k_radial_q"] = dict(flops=N * 2 * nR * KR * T, bytes=N * f4 * (T * KR + nR))
-    m["k_ang_fwd"] = dict(flops=PA * (GEO + basis(KA) + 2 * nA * KA + Y + 2 * NL * nA),
-                          bytes=16 * PA + N * f4 * (NL * nA + nA * nang))
+    # S1 (radial q from the aggregate B) runs inside k_ang_fwd
+    m["k_ang_fwd"] = dict(flops=PA * (GEO + basis(KA) + 2 * nA * KA + Y + 2 * NL * nA) + N * 2 * nR * KR * T,
+                          bytes=16 * PA + N * f4 * (NL * nA + nA * nang) + N * f4 * (T * KR + nR))
     m["k_ann_fwd"] = dict(flops=N * (4 * H * D + 6 * H + 2 * D + 2 * T * nR * KR),
                           bytes=N * f4 * (2 * D + H + T * KRP + 1))
     m["k_rad_force"] = dict(flops=PR * (GEO + basisd(KR) + 4 * KR + 22),
@@ -54,7 +54,7 @@ def kernel_models(model, sizes: dict) -> dict:
                               bytes=2 * 16 * PA + N * f4 * (2 * NL * nA + 2 * nA * nang + 3))
     npar = T * (D + 2) * H + 1 + T * T * (nR * KR + nA * KA)
     m["k_adam"] = dict(flops=12 * npar, bytes=7 * f4 * npar)
-    m["k_loss_atom"] = dict(flops=N * 12, bytes=N * f4 * 9)
+    m["k_loss"] = dict(flops=N * 12, bytes=N * f4 * 9)
     return m
 
 
