@@ -35,11 +35,13 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
         float* Gw = Gall + wib * TT * NK;
         float* pk = park + wib * WARP * PST;
         const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
-        float acc[NCH][K];
+        constexpr int KH = (K + 1) / 2;
+        float2 acc2[NCH][KH];   // (acc_n,2i, acc_n,2i+1); the odd tail pairs with a zero basis value
 #pragma unroll
         for (int n = 0; n < NCH; ++n)
 #pragma unroll
-            for (int k = 0; k < K; ++k) acc[n][k] = 0.0f;
+            for (int k = 0; k < KH; ++k) acc2[n][k] = make_float2(0.0f, 0.0f);
+        auto accv = [&](int n, int k) -> float& { return (k & 1) ? acc2[n][k >> 1].y : acc2[n][k >> 1].x; };
         int cur = -1;
         const int tiT = (L.ti > 0 ? L.ti : 0) * m.T;
         // parks the accumulators of the lanes whose run ended and adds them into the warp table (all lanes converged)
@@ -50,7 +52,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
 #pragma unroll
                 for (int n = 0; n < NCH; ++n)
 #pragma unroll
-                    for (int k = 0; k < K; ++k) { pk[L.lane * PST + n * K + k] = acc[n][k]; acc[n][k] = 0.0f; }
+                    for (int k = 0; k < K; ++k) { pk[L.lane * PST + n * K + k] = accv(n, k); accv(n, k) = 0.0f; }
             }
             __syncwarp();
             const int key = tiT + cur;
@@ -70,9 +72,10 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             cur = tj;
         };
         const float rcinv = m.rcinvA;
-        float X[NCH][NL];
+        float2 X2[NCH][NL / 2];
         // ---- pass 1: Sb ----
         {
+            float X[NCH][NL];
             const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
             const float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
             const float* Qbp = sb_ptr(a.b.Qb, L.w, m.D, L.lane);
@@ -92,27 +95,40 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
 #pragma unroll
                     for (int l = 0; l < NL; ++l) X[n][l] = 0.0f;
                 }
+                pack24(X[n], X2[n]);
             }
         }
         sweep_pairs(sw.rec, sw.width, sw.cnt, stage, pre, [&](const float4& rc4) {
             const PairGeo p = pair_geo(rc4);
             float b[NL], al[NCH];
+            float2 b2[NL / 2];
             harm24(harm_z(p.z), harm_xy(p.x, p.y), b);
+            pack24(b, b2);
 #pragma unroll
             for (int n = 0; n < NCH; ++n) {
-                float s1 = 0.0f;
+                float2 s1 = make_float2(0.0f, 0.0f);
 #pragma unroll
-                for (int l = 0; l < NL; ++l) s1 = fmaf(X[n][l], b[l], s1);
-                al[n] = s1;
+                for (int l = 0; l < NL / 2; ++l) s1 = __ffma2_rn(X2[n][l], b2[l], s1);
+                al[n] = s1.x + s1.y;
             }
-            cheb_basis<K, false>(p.r, rcinv, [&](int k, float fk, float) {
+            float fv[2 * KH];
+            fv[2 * KH - 1] = 0.0f;
+            cheb_basis<K, false>(p.r, rcinv, [&](int k, float fk, float) { fv[k] = fk; });
 #pragma unroll
-                for (int n = 0; n < NCH; ++n) acc[n][k] = fmaf(al[n], fk, acc[n][k]);
-            });
+            for (int n = 0; n < NCH; ++n) {
+                const float2 aa = dup2(al[n]);
+#pragma unroll
+                for (int k = 0; k < KH; ++k) acc2[n][k] = __ffma2_rn(aa, make_float2(fv[2 * k], fv[2 * k + 1]), acc2[n][k]);
+            }
         });
         if (multi) { flush(cur >= 0); cur = -1; }
         // ---- pass 2: EdS ----
-        load_EdS<NCH>(a, L, n0, X);
+        {
+            float X[NCH][NL];
+            load_EdS<NCH>(a, L, n0, X);
+#pragma unroll
+            for (int n = 0; n < NCH; ++n) pack24(X[n], X2[n]);
+        }
         float G[9];
 #pragma unroll
         for (int k = 0; k < 9; ++k) G[k] = __ldg(a.b.G + 9 * L.sb + k);
@@ -124,21 +140,29 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             const PairGeo p = pair_geo(rc4);
             const Tangent T = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
             float b[NL], bd[NL], be[NCH], de[NCH];
+            float2 b2[NL / 2], bd2[NL / 2];
             const HarmZ hz = harm_z(p.z);
             const HarmXY hxy = harm_xy(p.x, p.y);
             harm24(hz, hxy, b);
             harm24_tangent(hz, hxy, T.rx, T.ry, T.rz, bd);
+            pack24(b, b2); pack24(bd, bd2);
 #pragma unroll
             for (int n = 0; n < NCH; ++n) {
-                float s1 = 0.0f, s2 = 0.0f;
+                float2 s1 = make_float2(0.0f, 0.0f), s2 = make_float2(0.0f, 0.0f);
 #pragma unroll
-                for (int l = 0; l < NL; ++l) { s1 = fmaf(X[n][l], b[l], s1); s2 = fmaf(X[n][l], bd[l], s2); }
-                be[n] = s1 * T.t; de[n] = s2;
+                for (int l = 0; l < NL / 2; ++l) { s1 = __ffma2_rn(X2[n][l], b2[l], s1); s2 = __ffma2_rn(X2[n][l], bd2[l], s2); }
+                be[n] = (s1.x + s1.y) * T.t; de[n] = s2.x + s2.y;
             }
-            cheb_basis<K, true>(p.r, rcinv, [&](int k, float fk, float dfk) {
+            float fv[2 * KH], dfv[2 * KH];
+            fv[2 * KH - 1] = 0.0f; dfv[2 * KH - 1] = 0.0f;
+            cheb_basis<K, true>(p.r, rcinv, [&](int k, float fk, float dfk) { fv[k] = fk; dfv[k] = dfk; });
 #pragma unroll
-                for (int n = 0; n < NCH; ++n) acc[n][k] = fmaf(de[n], fk, fmaf(be[n], dfk, acc[n][k]));
-            });
+            for (int n = 0; n < NCH; ++n) {
+                const float2 dd = dup2(de[n]), bb = dup2(be[n]);
+#pragma unroll
+                for (int k = 0; k < KH; ++k)
+                    acc2[n][k] = __ffma2_rn(dd, make_float2(fv[2 * k], fv[2 * k + 1]), __ffma2_rn(bb, make_float2(dfv[2 * k], dfv[2 * k + 1]), acc2[n][k]));
+            }
         });
         if (multi) {
             flush(cur >= 0);
@@ -148,7 +172,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             for (int n = 0; n < NCH; ++n)
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    const float v = warp_sum(acc[n][k]);
+                    const float v = warp_sum(accv(n, k));
                     if (L.lane == 0) Gw[n * K + k] = v;
                 }
         }

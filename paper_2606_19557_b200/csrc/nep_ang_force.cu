@@ -19,8 +19,13 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
     Lane L;
     if (!lane_init(a, L)) return;
     const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
-    float EdS[NCH][NL];
-    load_EdS<NCH>(a, L, n0, EdS);
+    float2 E2[NCH][NL / 2];   // dE_i/dS in packed pairs
+    {
+        float EdS[NCH][NL];
+        load_EdS<NCH>(a, L, n0, EdS);
+#pragma unroll
+        for (int n = 0; n < NCH; ++n) pack24(EdS[n], E2[n]);
+    }
     float fx = 0.f, fy = 0.f, fz = 0.f, w[9];
 #pragma unroll
     for (int k = 0; k < 9; ++k) w[k] = 0.0f;
@@ -33,22 +38,26 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
         float g[NCH], dg[NCH];
         radial_gn<NCH, K, true>(p.r, rcinv, cbase + p.tj * CST, g, dg);
         float b[NL], A[NL];
+        float2 b2[NL / 2], A2[NL / 2];
         const HarmZ hz = harm_z(p.z);
         const HarmXY hxy = harm_xy(p.x, p.y);
         harm24(hz, hxy, b);
+        pack24(b, b2);
         float radial = 0.0f;
 #pragma unroll
-        for (int l = 0; l < NL; ++l) A[l] = 0.0f;
+        for (int l = 0; l < NL / 2; ++l) A2[l] = make_float2(0.0f, 0.0f);
 #pragma unroll
         for (int n = 0; n < NCH; ++n) {
-            float eb = 0.0f;
+            float2 eb = make_float2(0.0f, 0.0f);
+            const float2 gg = dup2(g[n]);
 #pragma unroll
-            for (int l = 0; l < NL; ++l) {
-                eb = fmaf(EdS[n][l], b[l], eb);
-                A[l] = fmaf(g[n], EdS[n][l], A[l]);
+            for (int l = 0; l < NL / 2; ++l) {
+                eb = __ffma2_rn(E2[n][l], b2[l], eb);
+                A2[l] = __ffma2_rn(gg, E2[n][l], A2[l]);
             }
-            radial = fmaf(dg[n], eb, radial);
+            radial = fmaf(dg[n], eb.x + eb.y, radial);
         }
+        unpack24(A2, A);
         float vx, vy, vz;
         harm24_grad_contract(hz, hxy, A, vx, vy, vz);
         const float vr = vx * p.x + vy * p.y + vz * p.z;

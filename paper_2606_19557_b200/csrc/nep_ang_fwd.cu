@@ -43,11 +43,11 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
 
     // ---- S2 ----
     const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
-    float S[NCH][NL];
+    float2 S2[NCH][NL / 2];   // (S_n,2i, S_n,2i+1): accumulated with packed FFMA2 (one issue slot per two lanes' FMAs)
 #pragma unroll
     for (int n = 0; n < NCH; ++n)
 #pragma unroll
-        for (int l = 0; l < NL; ++l) S[n][l] = 0.0f;
+        for (int l = 0; l < NL / 2; ++l) S2[n][l] = make_float2(0.0f, 0.0f);
     const float* cbase = cs + (L.ti > 0 ? L.ti : 0) * m.T * CST;
     const float rcinv = m.rcinvA;
     sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
@@ -59,10 +59,17 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
         const HarmXY hxy = harm_xy(p.x, p.y);
         harm24(hz, hxy, b);
 #pragma unroll
-        for (int n = 0; n < NCH; ++n)
+        for (int n = 0; n < NCH; ++n) {
+            const float2 gg = make_float2(g[n], g[n]);
 #pragma unroll
-            for (int l = 0; l < NL; ++l) S[n][l] = fmaf(g[n], b[l], S[n][l]);
+            for (int l = 0; l < NL / 2; ++l) S2[n][l] = __ffma2_rn(gg, make_float2(b[2 * l], b[2 * l + 1]), S2[n][l]);
+        }
     });
+    float S[NCH][NL];
+#pragma unroll
+    for (int n = 0; n < NCH; ++n)
+#pragma unroll
+        for (int l = 0; l < NL / 2; ++l) { S[n][2 * l] = S2[n][l].x; S[n][2 * l + 1] = S2[n][l].y; }
     float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
 #pragma unroll
     for (int n = 0; n < NCH; ++n) {

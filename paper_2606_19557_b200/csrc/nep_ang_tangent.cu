@@ -24,11 +24,11 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
     for (int k = 0; k < 9; ++k) G[k] = __ldg(a.b.G + 9 * L.sb + k);
     const float* ui = sb_ptr(a.b.u, L.w, 3, L.lane);
     const float uix = ui[0], uiy = ui[WARP], uiz = ui[2 * WARP];
-    float Sd[NCH][NL];
+    float2 Sd2[NCH][NL / 2];
 #pragma unroll
     for (int n = 0; n < NCH; ++n)
 #pragma unroll
-        for (int l = 0; l < NL; ++l) Sd[n][l] = 0.0f;
+        for (int l = 0; l < NL / 2; ++l) Sd2[n][l] = make_float2(0.0f, 0.0f);
     const float* cbase = cs + (L.ti > 0 ? L.ti : 0) * m.T * CST;
     const float rcinv = m.rcinvA;
     const float* ub = a.b.u;
@@ -43,13 +43,18 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
         const HarmXY hxy = harm_xy(p.x, p.y);
         harm24(hz, hxy, b);
         harm24_tangent(hz, hxy, T.rx, T.ry, T.rz, bd);
+        float2 b2[NL / 2], bd2[NL / 2];
+        pack24(b, b2); pack24(bd, bd2);
 #pragma unroll
         for (int n = 0; n < NCH; ++n) {
-            const float c1 = dg[n] * T.t;
+            const float2 cc = dup2(dg[n] * T.t), gg = dup2(g[n]);
 #pragma unroll
-            for (int l = 0; l < NL; ++l) Sd[n][l] = fmaf(c1, b[l], fmaf(g[n], bd[l], Sd[n][l]));
+            for (int l = 0; l < NL / 2; ++l) Sd2[n][l] = __ffma2_rn(cc, b2[l], __ffma2_rn(gg, bd2[l], Sd2[n][l]));
         }
     });
+    float Sd[NCH][NL];
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) unpack24(Sd2[n], Sd[n]);
     const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
     float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
     float* qdp = sb_ptr(a.b.qd, L.w, m.D, L.lane);

@@ -9,7 +9,7 @@
 //
 // The atoms of the batch are listed sorted by species (b.alist), every species padded to whole tiles of TM atoms, so
 // one tile sees ONE weight matrix and each contraction is a small dense fp32 GEMM out of shared memory:
-//   tile_gemm : [TM atoms] x [K] x [N outputs], thread = 8 atoms x up to 5 outputs in registers (FFMA : LDS = 40 : 7);
+//   tile_gemm : [TM atoms] x [K] x [N outputs], thread = AT (4 or 8) atoms x up to 5 outputs in registers;
 //   outer_gemm: sum over the TM atoms of outer products (the weight gradients), thread = 2 x up to 5 outputs.
 // fp32 FFMA on purpose: TF32/BF16 tensor-core inputs (10/7 mantissa bits) break the 1e-5 eV/atom energy tolerance and
 // the network is < 15 % of the step's arithmetic.
@@ -28,7 +28,7 @@ __host__ __device__ inline AnnLay ann_layout(const ModelDev& m, int TM, bool bwd
 {
     AnnLay l;
     l.TM = TM; l.LD = TM + 4;
-    l.DP8 = rup(m.D, 8); l.DPs = l.DP8 + 1; l.HP8 = rup(m.H, 8); l.HP16 = rup(m.H, TM / 8);
+    l.DP8 = rup(m.D, 8); l.DPs = l.DP8 + 1; l.HP8 = rup(m.H, 8); l.HP16 = rup(m.H, 32);   // rows of the outer-product GEMM: 32 row groups at most
     if (l.HP16 < l.HP8) l.HP16 = l.HP8;
     l.NH = l.HP8 / 8; l.NV = l.DP8 / 8;
     l.TK = m.T * m.KR; l.TKP = rup(m.T * m.KRP, 8); l.nR8 = rup(m.nR, 8);
@@ -46,7 +46,7 @@ __host__ __device__ inline AnnLay ann_layout(const ModelDev& m, int TM, bool bwd
         l.QDs = take(l.DP8 * l.LD);
         l.Gs = take(l.HP16 * l.LD);
         l.Bs = take(l.TK * l.LD); l.BDs = take(l.TK * l.LD); l.FPs = take(m.nR * l.LD);
-        l.red = take(2 * l.HP8 * (TM / 32));
+        l.red = take(2 * l.HP8 * 8);
     }
     l.total = o;
     return l;
@@ -73,27 +73,45 @@ __device__ __forceinline__ void for_chunks(int N, F&& f)
     }
 }
 
-// acc[i][j] = sum_k A[k * lda + i] * W[k * ldw + j * wstep],  i < 8 consecutive atoms, j < CW outputs
-template <int CW>
+// acc[i][j] = sum_k A[k * lda + i] * W[k * ldw + j * wstep],  i < AT consecutive atoms, j < CW outputs
+template <int AT, int CW>
 __device__ __forceinline__ void tile_gemm(const float* __restrict__ A, int lda, const float* __restrict__ W, int ldw, int wstep, int K,
-                                          float (&acc)[8][CW])
+                                          float (&acc)[AT][CW])
 {
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < AT; ++i)
 #pragma unroll
         for (int j = 0; j < CW; ++j) acc[i][j] = 0.0f;
-#pragma unroll 2
+#pragma unroll 4
     for (int k = 0; k < K; ++k) {
-        const float4 a0 = *reinterpret_cast<const float4*>(A + k * lda);
-        const float4 a1 = *reinterpret_cast<const float4*>(A + k * lda + 4);
-        const float av[8] = { a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w };
+        float av[AT];
+#pragma unroll
+        for (int i4 = 0; i4 < AT / 4; ++i4) {
+            const float4 a4 = *reinterpret_cast<const float4*>(A + k * lda + 4 * i4);
+            av[4 * i4] = a4.x; av[4 * i4 + 1] = a4.y; av[4 * i4 + 2] = a4.z; av[4 * i4 + 3] = a4.w;
+        }
         float w[CW];
 #pragma unroll
         for (int j = 0; j < CW; ++j) w[j] = W[k * ldw + j * wstep];
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < AT; ++i)
 #pragma unroll
             for (int j = 0; j < CW; ++j) acc[i][j] = fmaf(av[i], w[j], acc[i][j]);
+    }
+}
+template <int AT>
+__device__ __forceinline__ void store_atoms(float* dst, const float* v)
+{
+#pragma unroll
+    for (int i4 = 0; i4 < AT / 4; ++i4) reinterpret_cast<float4*>(dst)[i4] = make_float4(v[4 * i4], v[4 * i4 + 1], v[4 * i4 + 2], v[4 * i4 + 3]);
+}
+template <int AT>
+__device__ __forceinline__ void load_atoms(const float* src, float* v)
+{
+#pragma unroll
+    for (int i4 = 0; i4 < AT / 4; ++i4) {
+        const float4 a4 = reinterpret_cast<const float4*>(src)[i4];
+        v[4 * i4] = a4.x; v[4 * i4 + 1] = a4.y; v[4 * i4 + 2] = a4.z; v[4 * i4 + 3] = a4.w;
     }
 }
 
@@ -107,6 +125,7 @@ __device__ __forceinline__ void outer_gemm(const float* __restrict__ A1, const f
     for (int r = 0; r < RW; ++r)
 #pragma unroll
         for (int c = 0; c < CW; ++c) acc[r][c] = 0.0f;
+#pragma unroll 2
     for (int mm = 0; mm < TM; mm += 4) {
         float4 a1[RW], a2[RW], b1[CW], b2[CW];
 #pragma unroll
@@ -143,10 +162,8 @@ __device__ __forceinline__ void ann_load_weights(const StepArgs& a, const AnnLay
 {
     const ModelDev& m = a.m;
     const float* th = a.theta + (size_t)t * m.per_type;
-    for (int i = threadIdx.x; i < l.HP8 * l.DPs; i += blockDim.x) {
-        const int mu = i / l.DPs, v = i - mu * l.DPs;
-        sm[l.W0m + i] = (v < m.D && mu < m.H) ? th[mu * m.D + v] : 0.0f;
-    }
+    for (int mu = threadIdx.x / 32; mu < l.HP8; mu += blockDim.x / 32)
+        for (int v = threadIdx.x & 31; v < l.DPs; v += 32) sm[l.W0m + mu * l.DPs + v] = (v < m.D && mu < m.H) ? th[mu * m.D + v] : 0.0f;
     for (int i = threadIdx.x; i < l.HP8; i += blockDim.x) {
         if (want_b0) sm[l.b0 + i] = (i < m.H) ? th[m.H * m.D + i] : 0.0f;
         sm[l.w1 + i] = (i < m.H) ? th[m.H * m.D + m.H + i] : 0.0f;
@@ -154,68 +171,100 @@ __device__ __forceinline__ void ann_load_weights(const StepArgs& a, const AnnLay
     for (int i = threadIdx.x; i < l.DP8; i += blockDim.x) sm[l.sc + i] = (i < m.D) ? a.scaler[i] : 0.0f;
 }
 
+// Column gather: rows r = rg, rg + RG, ... < nrows of a slice-blocked array (src at row 0 of this atom, nullptr for a
+// padding atom) into dst[r * LD], optionally scaled by sc[r]; eight loads are issued before the first use.
+template <bool SCALE>
+__device__ __forceinline__ void gather_rows(float* __restrict__ dst, int LD, const float* __restrict__ src, int r0, int nrows, int rg, int RG,
+                                            const float* __restrict__ sc)
+{
+    for (int rb = r0 + rg; rb < nrows; rb += 8 * RG) {
+        float t[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int r = rb + j * RG;
+            t[j] = (src != nullptr && r < nrows) ? src[(size_t)r * WARP] : 0.0f;
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int r = rb + j * RG;
+            if (r < nrows) dst[r * LD] = SCALE ? t[j] * sc[r] : t[j];
+        }
+    }
+}
+__device__ __forceinline__ void scatter_rows(float* __restrict__ dst, const float* __restrict__ srcs, int LD, int r0, int nrows, int rg, int RG)
+{
+    for (int rb = r0 + rg; rb < nrows; rb += 8 * RG) {
+        float t[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int r = rb + j * RG;
+            t[j] = (r < nrows) ? srcs[r * LD] : 0.0f;
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int r = rb + j * RG;
+            if (r < nrows) dst[(size_t)r * WARP] = t[j];
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
-// S3
+// S3.  TM atoms per tile, AT atoms per thread: NT = 8 TM / AT threads; thread (ty, tx) = (atom group, output lane)
 // ------------------------------------------------------------------------------------------------
-template <int TM>
-__global__ void __launch_bounds__(TM) k_ann_fwd(StepArgs a)
+template <int TM, int AT>
+__global__ void __launch_bounds__(8 * TM / AT) k_ann_fwd(StepArgs a)
 {
     extern __shared__ __align__(16) float sm[];
+    constexpr int NT = 8 * TM / AT, RG = NT / TM;
     const ModelDev& m = a.m;
     const AnnLay l = ann_layout(m, TM, false);
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int t = tile_type(a.b, tile, m.T);
     ann_load_weights(a, l, sm, t, true);
-    for (int i = tid; i < m.nR * l.TKP; i += TM) {
+    for (int i = tid; i < m.nR * l.TKP; i += NT) {
         const int n = i / l.TKP, o = i - n * l.TKP, tj = o / m.KRP, k = o - tj * m.KRP;
         sm[l.cRs + i] = (tj < m.T && k < m.KR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
     }
     int* ibs = reinterpret_cast<int*>(sm + l.ibs);
-    const int ib = a.b.alist[(size_t)tile * TM + tid];
-    ibs[tid] = ib;
+    const int am = tid % TM, rg = tid / TM;          // gather role: atom am, row group rg
+    const int ib = a.b.alist[(size_t)tile * TM + am];
+    if (rg == 0) ibs[am] = ib;
     const int LD = l.LD;
     __syncthreads();
-    {   // gather q~ = s o q : thread = atom
-        float* Qm = sm + l.Qs + tid;
-        if (ib >= 0) {
-            const float* qp = sb_ptr(a.b.q, ib >> 5, m.D, ib & 31);
-            for (int v = 0; v < m.D; ++v) Qm[v * LD] = sm[l.sc + v] * qp[(size_t)v * WARP];
-        } else {
-            for (int v = 0; v < m.D; ++v) Qm[v * LD] = 0.0f;
-        }
-        for (int v = m.D; v < l.DP8; ++v) Qm[v * LD] = 0.0f;
+    {   // gather q~ = s o q
+        const float* qp = ib >= 0 ? sb_ptr(a.b.q, ib >> 5, m.D, ib & 31) : nullptr;
+        gather_rows<true>(sm + l.Qs + am, LD, qp, 0, m.D, rg, RG, sm + l.sc);
+        for (int v = m.D + rg; v < l.DP8; v += RG) sm[l.Qs + v * LD + am] = 0.0f;
     }
     __syncthreads();
-    const int ty = tid >> 3, tx = tid & 7, m0 = ty * 8;
-    float ei[8];
+    const int ty = tid >> 3, tx = tid & 7, m0 = ty * AT;
+    float ei[AT];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) ei[i] = 0.0f;
+    for (int i = 0; i < AT; ++i) ei[i] = 0.0f;
     float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TM;
     for_chunks(l.NH, [&](int j0, auto cwc) {
         constexpr int CW = decltype(cwc)::value;
-        float acc[8][CW];
-        tile_gemm<CW>(sm + l.Qs + m0, LD, sm + l.W0m + (tx + 8 * j0) * l.DPs, 1, 8 * l.DPs, m.D, acc);
+        float acc[AT][CW];
+        tile_gemm<AT, CW>(sm + l.Qs + m0, LD, sm + l.W0m + (tx + 8 * j0) * l.DPs, 1, 8 * l.DPs, m.D, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
             const int mu = tx + 8 * (j0 + j);
             const float b0 = sm[l.b0 + mu], w1 = sm[l.w1 + mu];
-            float h[8], e[8];
+            float h[AT], e[AT];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
+            for (int i = 0; i < AT; ++i) {
                 h[i] = tanhf(acc[i][j] - b0);
                 ei[i] = fmaf(w1, h[i], ei[i]);
                 e[i] = w1 * fmaf(-h[i], h[i], 1.0f);
             }
-            float4* es = reinterpret_cast<float4*>(sm + l.Es + mu * LD + m0);
-            es[0] = make_float4(e[0], e[1], e[2], e[3]); es[1] = make_float4(e[4], e[5], e[6], e[7]);
-            float4* hg = reinterpret_cast<float4*>(hb + (size_t)mu * TM + m0);
-            hg[0] = make_float4(h[0], h[1], h[2], h[3]); hg[1] = make_float4(h[4], h[5], h[6], h[7]);
+            store_atoms<AT>(sm + l.Es + mu * LD + m0, e);
+            store_atoms<AT>(hb + (size_t)mu * TM + m0, h);
         }
     });
     {   // E_i: sum over the 8 threads that share the atoms
         const float b1 = a.theta[m.o_b1];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < AT; ++i) {
             float v = ei[i];
             v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2); v += __shfl_xor_sync(0xffffffffu, v, 4);
             if (tx == 0) sm[l.aux + m0 + i] = v - b1;
@@ -225,32 +274,31 @@ __global__ void __launch_bounds__(TM) k_ann_fwd(StepArgs a)
     // Fp = s o (w0^T e), written over q~
     for_chunks(l.NV, [&](int j0, auto cwc) {
         constexpr int CW = decltype(cwc)::value;
-        float acc[8][CW];
-        tile_gemm<CW>(sm + l.Es + m0, LD, sm + l.W0m + tx + 8 * j0, l.DPs, 8, m.H, acc);
+        float acc[AT][CW];
+        tile_gemm<AT, CW>(sm + l.Es + m0, LD, sm + l.W0m + tx + 8 * j0, l.DPs, 8, m.H, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
             const int v = tx + 8 * (j0 + j);
             const float s = sm[l.sc + v];
-            float4* qs = reinterpret_cast<float4*>(sm + l.Qs + v * LD + m0);
-            qs[0] = make_float4(s * acc[0][j], s * acc[1][j], s * acc[2][j], s * acc[3][j]);
-            qs[1] = make_float4(s * acc[4][j], s * acc[5][j], s * acc[6][j], s * acc[7][j]);
+            float o[AT];
+#pragma unroll
+            for (int i = 0; i < AT; ++i) o[i] = s * acc[i][j];
+            store_atoms<AT>(sm + l.Qs + v * LD + m0, o);
         }
     });
     __syncthreads();
     if (ib >= 0) {
-        const float* Qm = sm + l.Qs + tid;
-        float* fp = sb_ptr(a.b.Fp, ib >> 5, m.D, ib & 31);
-        for (int v = 0; v < m.D; ++v) fp[(size_t)v * WARP] = Qm[v * LD];
-        a.b.Ei[ib] = sm[l.aux + tid];
+        scatter_rows(sb_ptr(a.b.Fp, ib >> 5, m.D, ib & 31), sm + l.Qs + am, LD, 0, m.D, rg, RG);
+        if (rg == 0) a.b.Ei[ib] = sm[l.aux + am];
     }
     // a_k[T'] = sum_n Fp_n cR[t][T'][n][k]
     const int TKRP = m.T * m.KRP;
     for_chunks(l.TKP / 8, [&](int j0, auto cwc) {
         constexpr int CW = decltype(cwc)::value;
-        float acc[8][CW];
-        tile_gemm<CW>(sm + l.Qs + m0, LD, sm + l.cRs + tx + 8 * j0, l.TKP, 8, m.nR, acc);
+        float acc[AT][CW];
+        tile_gemm<AT, CW>(sm + l.Qs + m0, LD, sm + l.cRs + tx + 8 * j0, l.TKP, 8, m.nR, acc);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < AT; ++i) {
             const int ibi = ibs[m0 + i];
             if (ibi < 0) continue;
             float* ar = a.b.arow + (size_t)ibi * TKRP;
@@ -266,93 +314,85 @@ __global__ void __launch_bounds__(TM) k_ann_fwd(StepArgs a)
 // ------------------------------------------------------------------------------------------------
 // S8
 // ------------------------------------------------------------------------------------------------
-template <int TM>
-__global__ void __launch_bounds__(TM) k_ann_bwd(StepArgs a)
+template <int TM, int AT>
+__global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
 {
     extern __shared__ __align__(16) float sm[];
+    constexpr int NT = 8 * TM / AT, RG = NT / TM, NW = NT / 32;
     const ModelDev& m = a.m;
     const AnnLay l = ann_layout(m, TM, true);
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int t = tile_type(a.b, tile, m.T);
-    constexpr int NW = TM / 32;
     ann_load_weights(a, l, sm, t, false);
-    for (int i = tid; i < l.TK * l.nR8; i += TM) {   // cRt[(tj, k)][n]
+    for (int i = tid; i < l.TK * l.nR8; i += NT) {   // cRt[(tj, k)][n]
         const int r = i / l.nR8, n = i - r * l.nR8, tj = r / m.KR, k = r - tj * m.KR;
         sm[l.cRt + i] = (n < m.nR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
     }
-    for (int i = tid; i < (l.HP16 - l.HP8) * l.LD; i += TM) { sm[l.Gs + l.HP8 * l.LD + i] = 0.0f; sm[l.Es + l.HP8 * l.LD + i] = 0.0f; }
+    for (int i = tid; i < (l.HP16 - l.HP8) * l.LD; i += NT) { sm[l.Gs + l.HP8 * l.LD + i] = 0.0f; sm[l.Es + l.HP8 * l.LD + i] = 0.0f; }
     int* ibs = reinterpret_cast<int*>(sm + l.ibs);
-    const int ib = a.b.alist[(size_t)tile * TM + tid];
-    ibs[tid] = ib;
+    const int am = tid % TM, rg = tid / TM;
+    const int ib = a.b.alist[(size_t)tile * TM + am];
+    if (rg == 0) ibs[am] = ib;
     const int LD = l.LD;
     __syncthreads();
-    {   // gather: thread = atom
-        float* Qm = sm + l.Qs + tid; float* QDm = sm + l.QDs + tid;
-        float* Bm = sm + l.Bs + tid; float* BDm = sm + l.BDs + tid; float* FPm = sm + l.FPs + tid;
+    {   // gather
+        const float *qp = nullptr, *qdp = nullptr, *fpp = nullptr, *Bp = nullptr, *Bdp = nullptr;
+        float epsi = 0.0f;
         if (ib >= 0) {
             const int w = ib >> 5, ln = ib & 31;
             const int4 bi = __ldg(a.b.binfo + w);
-            const float* qp = sb_ptr(a.b.q, w, m.D, ln);
-            const float* qdp = sb_ptr(a.b.qd, w, m.D, ln);
-            const float* fpp = sb_ptr(a.b.Fp, w, m.D, ln);
-            const float* Bp = sb_ptr(a.d.B, bi.x, l.TK, ln);
-            const float* Bdp = sb_ptr(a.b.Bd, w, l.TK, ln);
-            for (int v = 0; v < m.D; ++v) Qm[v * LD] = sm[l.sc + v] * qp[(size_t)v * WARP];
-            for (int v = m.nR; v < m.D; ++v) QDm[v * LD] = sm[l.sc + v] * qdp[(size_t)v * WARP];
-            for (int n = 0; n < m.nR; ++n) FPm[n * LD] = fpp[(size_t)n * WARP];
-            for (int r = 0; r < l.TK; ++r) { Bm[r * LD] = __ldg(Bp + (size_t)r * WARP); BDm[r * LD] = Bdp[(size_t)r * WARP]; }
-            sm[l.aux + tid] = a.b.eps[bi.y];
-        } else {
-            for (int v = 0; v < m.D; ++v) { Qm[v * LD] = 0.0f; QDm[v * LD] = 0.0f; }
-            for (int n = 0; n < m.nR; ++n) FPm[n * LD] = 0.0f;
-            for (int r = 0; r < l.TK; ++r) { Bm[r * LD] = 0.0f; BDm[r * LD] = 0.0f; }
-            sm[l.aux + tid] = 0.0f;
+            qp = sb_ptr(a.b.q, w, m.D, ln); qdp = sb_ptr(a.b.qd, w, m.D, ln); fpp = sb_ptr(a.b.Fp, w, m.D, ln);
+            Bp = sb_ptr(a.d.B, bi.x, l.TK, ln); Bdp = sb_ptr(a.b.Bd, w, l.TK, ln);
+            if (rg == 0) epsi = a.b.eps[bi.y];
         }
-        for (int v = m.D; v < l.DP8; ++v) { Qm[v * LD] = 0.0f; QDm[v * LD] = 0.0f; }
+        gather_rows<true>(sm + l.Qs + am, LD, qp, 0, m.D, rg, RG, sm + l.sc);
+        gather_rows<true>(sm + l.QDs + am, LD, qdp, m.nR, m.D, rg, RG, sm + l.sc);
+        gather_rows<false>(sm + l.FPs + am, LD, fpp, 0, m.nR, rg, RG, nullptr);
+        gather_rows<false>(sm + l.Bs + am, LD, Bp, 0, l.TK, rg, RG, nullptr);
+        gather_rows<false>(sm + l.BDs + am, LD, Bdp, 0, l.TK, rg, RG, nullptr);
+        if (rg == 0) sm[l.aux + am] = epsi;
+        for (int v = m.D + rg; v < l.DP8; v += RG) { sm[l.Qs + v * LD + am] = 0.0f; sm[l.QDs + v * LD + am] = 0.0f; }
     }
     __syncthreads();
-    const int ty = tid >> 3, tx = tid & 7, m0 = ty * 8;
+    const int ty = tid >> 3, tx = tid & 7, m0 = ty * AT;
     // radial tangent: qd_n = sum_{T', k} cR[t][T'][n][k] Bd_k[T'], scaled
     for_chunks(l.nR8 / 8, [&](int j0, auto cwc) {
         constexpr int CW = decltype(cwc)::value;
-        float acc[8][CW];
-        tile_gemm<CW>(sm + l.BDs + m0, LD, sm + l.cRt + tx + 8 * j0, l.nR8, 8, l.TK, acc);
+        float acc[AT][CW];
+        tile_gemm<AT, CW>(sm + l.BDs + m0, LD, sm + l.cRt + tx + 8 * j0, l.nR8, 8, l.TK, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
             const int n = tx + 8 * (j0 + j);
             if (n < m.nR) {
                 const float s = sm[l.sc + n];
-                float4* qd = reinterpret_cast<float4*>(sm + l.QDs + n * LD + m0);
-                qd[0] = make_float4(s * acc[0][j], s * acc[1][j], s * acc[2][j], s * acc[3][j]);
-                qd[1] = make_float4(s * acc[4][j], s * acc[5][j], s * acc[6][j], s * acc[7][j]);
+                float o[AT];
+#pragma unroll
+                for (int i = 0; i < AT; ++i) o[i] = s * acc[i][j];
+                store_atoms<AT>(sm + l.QDs + n * LD + m0, o);
             }
         }
     });
     __syncthreads();
     // xd = w0 (s o qd);  gamma, e, and the column sums for g_b0, g_w1
     const float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TM;
-    float epsv[8];
-    {
-        const float4 e0 = *reinterpret_cast<const float4*>(sm + l.aux + m0), e1 = *reinterpret_cast<const float4*>(sm + l.aux + m0 + 4);
-        epsv[0] = e0.x; epsv[1] = e0.y; epsv[2] = e0.z; epsv[3] = e0.w; epsv[4] = e1.x; epsv[5] = e1.y; epsv[6] = e1.z; epsv[7] = e1.w;
-    }
-    bool valid[8];
+    float epsv[AT];
+    load_atoms<AT>(sm + l.aux + m0, epsv);
+    bool valid[AT];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) valid[i] = ibs[m0 + i] >= 0;
+    for (int i = 0; i < AT; ++i) valid[i] = ibs[m0 + i] >= 0;
     for_chunks(l.NH, [&](int j0, auto cwc) {
         constexpr int CW = decltype(cwc)::value;
-        float acc[8][CW];
-        tile_gemm<CW>(sm + l.QDs + m0, LD, sm + l.W0m + (tx + 8 * j0) * l.DPs, 1, 8 * l.DPs, m.D, acc);
+        float acc[AT][CW];
+        tile_gemm<AT, CW>(sm + l.QDs + m0, LD, sm + l.W0m + (tx + 8 * j0) * l.DPs, 1, 8 * l.DPs, m.D, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
             const int mu = tx + 8 * (j0 + j);
             const float w1 = sm[l.w1 + mu];
-            const float4 h0 = *reinterpret_cast<const float4*>(hb + (size_t)mu * TM + m0);
-            const float4 h1 = *reinterpret_cast<const float4*>(hb + (size_t)mu * TM + m0 + 4);
-            const float h[8] = { h0.x, h0.y, h0.z, h0.w, h1.x, h1.y, h1.z, h1.w };
-            float gam[8], e[8], sg = 0.0f, sw = 0.0f;
+            float h[AT];
+            load_atoms<AT>(hb + (size_t)mu * TM + m0, h);
+            float gam[AT], e[AT], sg = 0.0f, sw = 0.0f;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
+            for (int i = 0; i < AT; ++i) {
                 const float omh2 = fmaf(-h[i], h[i], 1.0f);
                 const float ee = valid[i] ? w1 * omh2 : 0.0f;
                 const float xd = acc[i][j];
@@ -361,10 +401,8 @@ __global__ void __launch_bounds__(TM) k_ann_bwd(StepArgs a)
                 sg += gam[i];
                 sw += valid[i] ? fmaf(epsv[i], h[i], omh2 * xd) : 0.0f;
             }
-            float4* gs = reinterpret_cast<float4*>(sm + l.Gs + mu * LD + m0);
-            gs[0] = make_float4(gam[0], gam[1], gam[2], gam[3]); gs[1] = make_float4(gam[4], gam[5], gam[6], gam[7]);
-            float4* es = reinterpret_cast<float4*>(sm + l.Es + mu * LD + m0);
-            es[0] = make_float4(e[0], e[1], e[2], e[3]); es[1] = make_float4(e[4], e[5], e[6], e[7]);
+            store_atoms<AT>(sm + l.Gs + mu * LD + m0, gam);
+            store_atoms<AT>(sm + l.Es + mu * LD + m0, e);
             // sum over the 4 atom groups of this warp (lanes with equal tx), then across warps through shared memory
             sg += __shfl_xor_sync(0xffffffffu, sg, 8); sg += __shfl_xor_sync(0xffffffffu, sg, 16);
             sw += __shfl_xor_sync(0xffffffffu, sw, 8); sw += __shfl_xor_sync(0xffffffffu, sw, 16);
@@ -377,7 +415,7 @@ __global__ void __launch_bounds__(TM) k_ann_bwd(StepArgs a)
     __syncthreads();
     {   // g_b0[t][mu] -= sum gamma ; g_w1[t][mu] += sum (eps h + (1-h^2) xd)
         float* gt = a.g + (size_t)t * m.per_type + m.H * m.D;
-        for (int i = tid; i < 2 * m.H; i += TM) {
+        for (int i = tid; i < 2 * m.H; i += NT) {
             const int which = i / m.H, mu = i - which * m.H;
             float s = 0.0f;
 #pragma unroll
@@ -386,11 +424,12 @@ __global__ void __launch_bounds__(TM) k_ann_bwd(StepArgs a)
         }
     }
     {   // g_w0[t][mu][v] += sum_atoms gamma_mu q~_v + e_mu (s qd)_v : thread = rows {ra + RS jr} x cols {cb + 8 jc}
-        constexpr int RS = TM / 8;
+        constexpr int RS = NT / 8;
         const int ra = tid >> 3, cb = tid & 7;
         float* gt = a.g + (size_t)t * m.per_type;
-        for (int jr0 = 0; jr0 < l.HP16 / RS; jr0 += 2) {
-            const bool two = jr0 + 1 < l.HP16 / RS;
+        const int nrg = (l.HP8 + RS - 1) / RS;          // row groups that hold real rows (rows up to HP16 are zero)
+        for (int jr0 = 0; jr0 < nrg; jr0 += 2) {
+            const bool two = jr0 + 1 < nrg;
             const int r0 = ra + RS * jr0;
             for_chunks(l.NV, [&](int jc0, auto cwc) {
                 constexpr int CW = decltype(cwc)::value;
@@ -421,25 +460,22 @@ __global__ void __launch_bounds__(TM) k_ann_bwd(StepArgs a)
     // Qb = s o (w0^T gamma), written over q~
     for_chunks(l.NV, [&](int j0, auto cwc) {
         constexpr int CW = decltype(cwc)::value;
-        float acc[8][CW];
-        tile_gemm<CW>(sm + l.Gs + m0, LD, sm + l.W0m + tx + 8 * j0, l.DPs, 8, m.H, acc);
+        float acc[AT][CW];
+        tile_gemm<AT, CW>(sm + l.Gs + m0, LD, sm + l.W0m + tx + 8 * j0, l.DPs, 8, m.H, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
             const int v = tx + 8 * (j0 + j);
             const float s = sm[l.sc + v];
-            float4* qs = reinterpret_cast<float4*>(sm + l.Qs + v * LD + m0);
-            qs[0] = make_float4(s * acc[0][j], s * acc[1][j], s * acc[2][j], s * acc[3][j]);
-            qs[1] = make_float4(s * acc[4][j], s * acc[5][j], s * acc[6][j], s * acc[7][j]);
+            float o[AT];
+#pragma unroll
+            for (int i = 0; i < AT; ++i) o[i] = s * acc[i][j];
+            store_atoms<AT>(sm + l.Qs + v * LD + m0, o);
         }
     });
     __syncthreads();
-    if (ib >= 0) {
-        const float* Qm = sm + l.Qs + tid;
-        float* qb = sb_ptr(a.b.Qb, ib >> 5, m.D, ib & 31);
-        for (int v = m.nR; v < m.D; ++v) qb[(size_t)v * WARP] = Qm[v * LD];   // only the angular rows are read later
-    }
+    if (ib >= 0) scatter_rows(sb_ptr(a.b.Qb, ib >> 5, m.D, ib & 31), sm + l.Qs + am, LD, m.nR, m.D, rg, RG);   // only the angular rows are read later
     // g_cR[t][T'][n][k] += sum_atoms Qb_n B_k[T'] + Fp_n Bd_k[T'] : one output per thread
-    for (int o = tid; o < m.nR * l.TK; o += TM) {
+    for (int o = tid; o < m.nR * l.TK; o += NT) {
         const int n = o / l.TK, r = o - n * l.TK;
         float acc[1][1];
         outer_gemm<1, 1>(sm + l.Qs + n * LD, sm + l.FPs + n * LD, 0, sm + l.Bs + r * LD, sm + l.BDs + r * LD, 0, TM, acc);
@@ -451,6 +487,8 @@ __global__ void __launch_bounds__(TM) k_ann_bwd(StepArgs a)
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
+constexpr int ANN_AT = 4;   // atoms per thread: 256 threads per 128-atom tile
+
 int ann_tile_m(const nep_ctx* c)
 {
     // 128-atom tiles while two blocks of the larger (backward) kernel fit in one SM's shared memory, else 64
@@ -461,15 +499,16 @@ int ann_tile_m(const nep_ctx* c)
 template <int TM>
 static int launch_ann_t(nep_ctx* c, const StepArgs& a, bool bwd)
 {
+    constexpr int NT = 8 * TM / ANN_AT;
     const size_t smem = 4 * (size_t)ann_layout(c->m, TM, bwd).total;
     if (smem > (size_t)c->max_smem_optin) return fail(c, NEP_ECAPACITY, "network tile does not fit in shared memory (neurons x descriptors too large)");
     if (c->b.ntiles == 0) return NEP_OK;
     if (bwd) {
-        NEP_CUDA(c, cudaFuncSetAttribute(k_ann_bwd<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        NEP_LAUNCH(c, "k_ann_bwd", k_ann_bwd<TM>, c->b.ntiles, TM, smem, a);
+        NEP_CUDA(c, cudaFuncSetAttribute(k_ann_bwd<TM, ANN_AT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NEP_LAUNCH(c, "k_ann_bwd", (k_ann_bwd<TM, ANN_AT>), c->b.ntiles, NT, smem, a);
     } else {
-        NEP_CUDA(c, cudaFuncSetAttribute(k_ann_fwd<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        NEP_LAUNCH(c, "k_ann_fwd", k_ann_fwd<TM>, c->b.ntiles, TM, smem, a);
+        NEP_CUDA(c, cudaFuncSetAttribute(k_ann_fwd<TM, ANN_AT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NEP_LAUNCH(c, "k_ann_fwd", (k_ann_fwd<TM, ANN_AT>), c->b.ntiles, NT, smem, a);
     }
     return NEP_OK;
 }

@@ -210,6 +210,19 @@ __device__ __forceinline__ void store_inv(const ModelDev& m, float* __restrict__
     if (m.has5) arr[(size_t)ang_row(m, 5, n) * WARP] = q[5];
 }
 
+// packed pairs: two fp32 lanes of work per issue slot (FFMA2 on sm_100)
+__device__ __forceinline__ float2 dup2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ void pack24(const float* b, float2* b2)
+{
+#pragma unroll
+    for (int i = 0; i < NL / 2; ++i) b2[i] = make_float2(b[2 * i], b[2 * i + 1]);
+}
+__device__ __forceinline__ void unpack24(const float2* b2, float* b)
+{
+#pragma unroll
+    for (int i = 0; i < NL / 2; ++i) { b[2 * i] = b2[i].x; b[2 * i + 1] = b2[i].y; }
+}
+
 // EdS_nL = dE_i/dS_nL = sum_a Fp[q index (a, n)] dq_a/dS_nL for the NCH channels of this thread (DESIGN C8)
 template <int NCH>
 __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n0, float (*EdS)[NL])
