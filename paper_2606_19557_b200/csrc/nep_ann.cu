@@ -9,10 +9,13 @@
 //
 // The atoms of the batch are listed sorted by species (b.alist), every species padded to whole tiles of TM atoms, so
 // one tile sees ONE weight matrix and each contraction is a small dense fp32 GEMM out of shared memory:
-//   tile_gemm : [TM atoms] x [K] x [N outputs], thread = AT (4 or 8) atoms x up to 5 outputs in registers;
-//   outer_gemm: sum over the TM atoms of outer products (the weight gradients), thread = 2 x up to 5 outputs.
+//   tile_gemm : [TM atoms] x [K] x [N outputs]; thread = AT atoms x 4 outputs, both operands fetched with one LDS.128
+//               per k (16 FFMA per 2 LDS); outputs beyond a multiple of 32 use a strided scalar tail;
+//   outer_gemm: sum over the TM atoms of outer products (the weight gradients).
+// The descriptor scaler (Eq. 2) is folded into the weights held in shared memory, W0s[mu][v] = w0[mu][v] s_v, so the
+// per-atom inputs are copied global -> shared unchanged with cp.async (all rows of a tile in flight at once).
 // fp32 FFMA on purpose: TF32/BF16 tensor-core inputs (10/7 mantissa bits) break the 1e-5 eV/atom energy tolerance and
-// the network is < 15 % of the step's arithmetic.
+// the network is a small part of the step's arithmetic.
 #include <type_traits>
 
 #include "nep_kernels.cuh"
@@ -20,31 +23,30 @@
 namespace nep {
 
 struct AnnLay {
-    int TM, LD, DP8, DPs, HP8, HP16, NH, NV, TK, TKP, nR8;
-    int W0m, b0, w1, sc, cRs, cRt, Qs, QDs, Gs, Es, Bs, BDs, FPs, ibs, aux, red, total;   // float offsets
+    int TM, LD, DP8, HP8, HP32, TK, TKP, nR8;
+    int W0m, W0t, b0, w1, sc, cRs, cRt, Qs, QDs, Gs, Es, Bs, BDs, FPs, ibs, aux, red, total;   // float offsets
 };
 __host__ __device__ inline int rup(int x, int m) { return (x + m - 1) / m * m; }
 __host__ __device__ inline AnnLay ann_layout(const ModelDev& m, int TM, bool bwd)
 {
     AnnLay l;
     l.TM = TM; l.LD = TM + 4;
-    l.DP8 = rup(m.D, 8); l.DPs = l.DP8 + 1; l.HP8 = rup(m.H, 8); l.HP16 = rup(m.H, 32);   // rows of the outer-product GEMM: 32 row groups at most
-    if (l.HP16 < l.HP8) l.HP16 = l.HP8;
-    l.NH = l.HP8 / 8; l.NV = l.DP8 / 8;
+    l.DP8 = rup(m.D, 8); l.HP8 = rup(m.H, 8); l.HP32 = rup(m.H, 32);   // HP32: rows of the outer-product GEMM (zero padded)
     l.TK = m.T * m.KR; l.TKP = rup(m.T * m.KRP, 8); l.nR8 = rup(m.nR, 8);
     int o = 0;
     auto take = [&](int n) { int r = o; o += rup(n, 4); return r; };
-    l.W0m = take(l.HP8 * l.DPs); l.b0 = take(l.HP8); l.w1 = take(l.HP8); l.sc = take(l.DP8);
+    l.W0m = take(l.HP8 * l.DP8); l.W0t = take(l.DP8 * l.HP8);
+    l.b0 = take(l.HP8); l.w1 = take(l.HP8); l.sc = take(l.DP8);
     l.cRs = l.cRt = l.QDs = l.Gs = l.Bs = l.BDs = l.FPs = l.red = 0;
     l.Qs = take(l.DP8 * l.LD);
-    l.Es = take(l.HP16 * l.LD);
+    l.Es = take(l.HP32 * l.LD);
     l.ibs = take(TM); l.aux = take(TM);
     if (!bwd) {
         l.cRs = take(m.nR * l.TKP);
     } else {
         l.cRt = take(l.TK * l.nR8);
         l.QDs = take(l.DP8 * l.LD);
-        l.Gs = take(l.HP16 * l.LD);
+        l.Gs = take(l.HP32 * l.LD);
         l.Bs = take(l.TK * l.LD); l.BDs = take(l.TK * l.LD); l.FPs = take(m.nR * l.LD);
         l.red = take(2 * l.HP8 * 8);
     }
@@ -52,30 +54,26 @@ __host__ __device__ inline AnnLay ann_layout(const ModelDev& m, int TM, bool bwd
     return l;
 }
 
-// splits N outputs-per-thread into ceil(N/5) nearly equal chunks and calls f(first, integral_constant<width>)
+// Outputs of one thread (lane tx of 8) among n_out (a multiple of 8): rounds of 32 as quads {32c + 4tx + j}, then a
+// strided tail {32C + tx + 8j}.  f(o0, ostep, integral_constant<CW>, integral_constant<QUAD>)
 template <class F>
-__device__ __forceinline__ void for_chunks(int N, F&& f)
+__device__ __forceinline__ void for_outputs(int n_out, int tx, F&& f)
 {
-    const int chunks = (N + 4) / 5;
-    if (chunks == 0) return;
-    const int base = N / chunks, rem = N - base * chunks;
-    int j0 = 0;
-    for (int c = 0; c < chunks; ++c) {
-        const int cw = base + (c < rem ? 1 : 0);
-        switch (cw) {
-        case 1: f(j0, std::integral_constant<int, 1>{}); break;
-        case 2: f(j0, std::integral_constant<int, 2>{}); break;
-        case 3: f(j0, std::integral_constant<int, 3>{}); break;
-        case 4: f(j0, std::integral_constant<int, 4>{}); break;
-        default: f(j0, std::integral_constant<int, 5>{}); break;
-        }
-        j0 += cw;
+    const int C = n_out >> 5, rem = (n_out & 31) >> 3;
+    for (int c = 0; c < C; ++c) f(32 * c + 4 * tx, 1, std::integral_constant<int, 4>{}, std::true_type{});
+    const int o0 = 32 * C + tx;
+    switch (rem) {
+    case 1: f(o0, 8, std::integral_constant<int, 1>{}, std::false_type{}); break;
+    case 2: f(o0, 8, std::integral_constant<int, 2>{}, std::false_type{}); break;
+    case 3: f(o0, 8, std::integral_constant<int, 3>{}, std::false_type{}); break;
+    default: break;
     }
 }
 
-// acc[i][j] = sum_k A[k * lda + i] * W[k * ldw + j * wstep],  i < AT consecutive atoms, j < CW outputs
-template <int AT, int CW>
-__device__ __forceinline__ void tile_gemm(const float* __restrict__ A, int lda, const float* __restrict__ W, int ldw, int wstep, int K,
+// acc[i][j] = sum_k A[k * lda + i] * W[k * ldw + j * ostep],  i < AT consecutive atoms, j < CW outputs
+// (QUAD: ostep == 1 and the four weights are one 128-bit load)
+template <int AT, int CW, bool QUAD>
+__device__ __forceinline__ void tile_gemm(const float* __restrict__ A, int lda, const float* __restrict__ W, int ldw, int ostep, int K,
                                           float (&acc)[AT][CW])
 {
 #pragma unroll
@@ -91,8 +89,13 @@ __device__ __forceinline__ void tile_gemm(const float* __restrict__ A, int lda, 
             av[4 * i4] = a4.x; av[4 * i4 + 1] = a4.y; av[4 * i4 + 2] = a4.z; av[4 * i4 + 3] = a4.w;
         }
         float w[CW];
+        if (QUAD) {
+            const float4 w4 = *reinterpret_cast<const float4*>(W + k * ldw);
+            w[0] = w4.x; if (CW > 1) w[1] = w4.y; if (CW > 2) w[2] = w4.z; if (CW > 3) w[3] = w4.w;
+        } else {
 #pragma unroll
-        for (int j = 0; j < CW; ++j) w[j] = W[k * ldw + j * wstep];
+            for (int j = 0; j < CW; ++j) w[j] = W[k * ldw + j * ostep];
+        }
 #pragma unroll
         for (int i = 0; i < AT; ++i)
 #pragma unroll
@@ -149,6 +152,26 @@ __device__ __forceinline__ void outer_gemm(const float* __restrict__ A1, const f
             }
     }
 }
+// splits N column groups into ceil(N/5) nearly equal chunks: f(first, integral_constant<width>)
+template <class F>
+__device__ __forceinline__ void for_chunks(int N, F&& f)
+{
+    const int chunks = (N + 4) / 5;
+    if (chunks == 0) return;
+    const int base = N / chunks, rem = N - base * chunks;
+    int j0 = 0;
+    for (int c = 0; c < chunks; ++c) {
+        const int cw = base + (c < rem ? 1 : 0);
+        switch (cw) {
+        case 1: f(j0, std::integral_constant<int, 1>{}); break;
+        case 2: f(j0, std::integral_constant<int, 2>{}); break;
+        case 3: f(j0, std::integral_constant<int, 3>{}); break;
+        case 4: f(j0, std::integral_constant<int, 4>{}); break;
+        default: f(j0, std::integral_constant<int, 5>{}); break;
+        }
+        j0 += cw;
+    }
+}
 
 __device__ __forceinline__ int tile_type(const BatchDev& b, int tile, int T)
 {
@@ -157,13 +180,18 @@ __device__ __forceinline__ int tile_type(const BatchDev& b, int tile, int T)
     return t;
 }
 
-// weights of species t into shared memory (zero padded): W0m[mu][v] (row stride DPs, odd), b0, w1, scaler
+// weights of species t into shared memory, zero padded and with the scaler folded in:
+// W0m[mu][v] = W0t[v][mu] = w0[mu][v] s_v;  b0, w1, scaler
 __device__ __forceinline__ void ann_load_weights(const StepArgs& a, const AnnLay& l, float* sm, int t, bool want_b0)
 {
     const ModelDev& m = a.m;
     const float* th = a.theta + (size_t)t * m.per_type;
     for (int mu = threadIdx.x / 32; mu < l.HP8; mu += blockDim.x / 32)
-        for (int v = threadIdx.x & 31; v < l.DPs; v += 32) sm[l.W0m + mu * l.DPs + v] = (v < m.D && mu < m.H) ? th[mu * m.D + v] : 0.0f;
+        for (int v = threadIdx.x & 31; v < l.DP8; v += 32) {
+            const float w = (v < m.D && mu < m.H) ? th[mu * m.D + v] * a.scaler[v] : 0.0f;
+            sm[l.W0m + mu * l.DP8 + v] = w;
+            sm[l.W0t + v * l.HP8 + mu] = w;
+        }
     for (int i = threadIdx.x; i < l.HP8; i += blockDim.x) {
         if (want_b0) sm[l.b0 + i] = (i < m.H) ? th[m.H * m.D + i] : 0.0f;
         sm[l.w1 + i] = (i < m.H) ? th[m.H * m.D + m.H + i] : 0.0f;
@@ -171,24 +199,19 @@ __device__ __forceinline__ void ann_load_weights(const StepArgs& a, const AnnLay
     for (int i = threadIdx.x; i < l.DP8; i += blockDim.x) sm[l.sc + i] = (i < m.D) ? a.scaler[i] : 0.0f;
 }
 
-// Column gather: rows r = rg, rg + RG, ... < nrows of a slice-blocked array (src at row 0 of this atom, nullptr for a
-// padding atom) into dst[r * LD], optionally scaled by sc[r]; eight loads are issued before the first use.
-template <bool SCALE>
-__device__ __forceinline__ void gather_rows(float* __restrict__ dst, int LD, const float* __restrict__ src, int r0, int nrows, int rg, int RG,
-                                            const float* __restrict__ sc)
+__device__ __forceinline__ void cp_async4(float* smem_dst, const float* gsrc)
 {
-    for (int rb = r0 + rg; rb < nrows; rb += 8 * RG) {
-        float t[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int r = rb + j * RG;
-            t[j] = (src != nullptr && r < nrows) ? src[(size_t)r * WARP] : 0.0f;
-        }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int r = rb + j * RG;
-            if (r < nrows) dst[r * LD] = SCALE ? t[j] * sc[r] : t[j];
-        }
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(s), "l"(gsrc) : "memory");
+}
+// Column gather: rows r = r0 + rg, + RG, ... < nrows of a slice-blocked array (src at row 0 of this atom; nullptr for
+// a padding atom: zeros) into dst[r * LD], asynchronously (cp.async; the caller commits and waits).
+__device__ __forceinline__ void gather_rows(float* __restrict__ dst, int LD, const float* __restrict__ src, int r0, int nrows, int rg, int RG)
+{
+    if (src != nullptr) {
+        for (int r = r0 + rg; r < nrows; r += RG) cp_async4(dst + r * LD, src + (size_t)r * WARP);
+    } else {
+        for (int r = r0 + rg; r < nrows; r += RG) dst[r * LD] = 0.0f;
     }
 }
 __device__ __forceinline__ void scatter_rows(float* __restrict__ dst, const float* __restrict__ srcs, int LD, int r0, int nrows, int rg, int RG)
@@ -219,36 +242,38 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_fwd(StepArgs a)
     const ModelDev& m = a.m;
     const AnnLay l = ann_layout(m, TM, false);
     const int tile = blockIdx.x, tid = threadIdx.x;
+    const int LD = l.LD;
+    int* ibs = reinterpret_cast<int*>(sm + l.ibs);
+    const int am = tid % TM, rg = tid / TM;          // gather role: atom am, row group rg
+    const int ib = a.b.alist[(size_t)tile * TM + am];
+    {   // q of the tile, unscaled, straight into shared memory
+        const float* qp = ib >= 0 ? sb_ptr(a.b.q, ib >> 5, m.D, ib & 31) : nullptr;
+        gather_rows(sm + l.Qs + am, LD, qp, 0, m.D, rg, RG);
+        cp_async_commit();
+        for (int v = m.D + rg; v < l.DP8; v += RG) sm[l.Qs + v * LD + am] = 0.0f;
+        if (rg == 0) ibs[am] = ib;
+    }
     const int t = tile_type(a.b, tile, m.T);
     ann_load_weights(a, l, sm, t, true);
     for (int i = tid; i < m.nR * l.TKP; i += NT) {
         const int n = i / l.TKP, o = i - n * l.TKP, tj = o / m.KRP, k = o - tj * m.KRP;
         sm[l.cRs + i] = (tj < m.T && k < m.KR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
     }
-    int* ibs = reinterpret_cast<int*>(sm + l.ibs);
-    const int am = tid % TM, rg = tid / TM;          // gather role: atom am, row group rg
-    const int ib = a.b.alist[(size_t)tile * TM + am];
-    if (rg == 0) ibs[am] = ib;
-    const int LD = l.LD;
-    __syncthreads();
-    {   // gather q~ = s o q
-        const float* qp = ib >= 0 ? sb_ptr(a.b.q, ib >> 5, m.D, ib & 31) : nullptr;
-        gather_rows<true>(sm + l.Qs + am, LD, qp, 0, m.D, rg, RG, sm + l.sc);
-        for (int v = m.D + rg; v < l.DP8; v += RG) sm[l.Qs + v * LD + am] = 0.0f;
-    }
+    cp_async_wait<0>();
     __syncthreads();
     const int ty = tid >> 3, tx = tid & 7, m0 = ty * AT;
     float ei[AT];
 #pragma unroll
     for (int i = 0; i < AT; ++i) ei[i] = 0.0f;
     float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TM;
-    for_chunks(l.NH, [&](int j0, auto cwc) {
+    for_outputs(l.HP8, tx, [&](int o0, int ostep, auto cwc, auto quadc) {
         constexpr int CW = decltype(cwc)::value;
+        constexpr bool QUAD = decltype(quadc)::value;
         float acc[AT][CW];
-        tile_gemm<AT, CW>(sm + l.Qs + m0, LD, sm + l.W0m + (tx + 8 * j0) * l.DPs, 1, 8 * l.DPs, m.D, acc);
+        tile_gemm<AT, CW, QUAD>(sm + l.Qs + m0, LD, sm + l.W0t + o0, l.HP8, ostep, m.D, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
-            const int mu = tx + 8 * (j0 + j);
+            const int mu = o0 + j * ostep;
             const float b0 = sm[l.b0 + mu], w1 = sm[l.w1 + mu];
             float h[AT], e[AT];
 #pragma unroll
@@ -271,19 +296,18 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_fwd(StepArgs a)
         }
     }
     __syncthreads();
-    // Fp = s o (w0^T e), written over q~
-    for_chunks(l.NV, [&](int j0, auto cwc) {
+    // Fp = s o (w0^T e), written over q
+    for_outputs(l.DP8, tx, [&](int o0, int ostep, auto cwc, auto quadc) {
         constexpr int CW = decltype(cwc)::value;
+        constexpr bool QUAD = decltype(quadc)::value;
         float acc[AT][CW];
-        tile_gemm<AT, CW>(sm + l.Es + m0, LD, sm + l.W0m + tx + 8 * j0, l.DPs, 8, m.H, acc);
+        tile_gemm<AT, CW, QUAD>(sm + l.Es + m0, LD, sm + l.W0m + o0, l.DP8, ostep, m.H, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
-            const int v = tx + 8 * (j0 + j);
-            const float s = sm[l.sc + v];
             float o[AT];
 #pragma unroll
-            for (int i = 0; i < AT; ++i) o[i] = s * acc[i][j];
-            store_atoms<AT>(sm + l.Qs + v * LD + m0, o);
+            for (int i = 0; i < AT; ++i) o[i] = acc[i][j];
+            store_atoms<AT>(sm + l.Qs + (o0 + j * ostep) * LD + m0, o);
         }
     });
     __syncthreads();
@@ -293,19 +317,24 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_fwd(StepArgs a)
     }
     // a_k[T'] = sum_n Fp_n cR[t][T'][n][k]
     const int TKRP = m.T * m.KRP;
-    for_chunks(l.TKP / 8, [&](int j0, auto cwc) {
+    for_outputs(l.TKP, tx, [&](int o0, int ostep, auto cwc, auto quadc) {
         constexpr int CW = decltype(cwc)::value;
+        constexpr bool QUAD = decltype(quadc)::value;
         float acc[AT][CW];
-        tile_gemm<AT, CW>(sm + l.Qs + m0, LD, sm + l.cRs + tx + 8 * j0, l.TKP, 8, m.nR, acc);
+        tile_gemm<AT, CW, QUAD>(sm + l.Qs + m0, LD, sm + l.cRs + o0, l.TKP, ostep, m.nR, acc);
 #pragma unroll
         for (int i = 0; i < AT; ++i) {
             const int ibi = ibs[m0 + i];
             if (ibi < 0) continue;
             float* ar = a.b.arow + (size_t)ibi * TKRP;
+            if (QUAD && o0 + 3 < TKRP) {
+                *reinterpret_cast<float4*>(ar + o0) = make_float4(acc[i][0], acc[i][CW > 1 ? 1 : 0], acc[i][CW > 2 ? 2 : 0], acc[i][CW > 3 ? 3 : 0]);
+            } else {
 #pragma unroll
-            for (int j = 0; j < CW; ++j) {
-                const int o = tx + 8 * (j0 + j);
-                if (o < TKRP) ar[o] = acc[i][j];
+                for (int j = 0; j < CW; ++j) {
+                    const int o = o0 + j * ostep;
+                    if (o < TKRP) ar[o] = acc[i][j];
+                }
             }
         }
     });
@@ -322,20 +351,11 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
     const ModelDev& m = a.m;
     const AnnLay l = ann_layout(m, TM, true);
     const int tile = blockIdx.x, tid = threadIdx.x;
-    const int t = tile_type(a.b, tile, m.T);
-    ann_load_weights(a, l, sm, t, false);
-    for (int i = tid; i < l.TK * l.nR8; i += NT) {   // cRt[(tj, k)][n]
-        const int r = i / l.nR8, n = i - r * l.nR8, tj = r / m.KR, k = r - tj * m.KR;
-        sm[l.cRt + i] = (n < m.nR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
-    }
-    for (int i = tid; i < (l.HP16 - l.HP8) * l.LD; i += NT) { sm[l.Gs + l.HP8 * l.LD + i] = 0.0f; sm[l.Es + l.HP8 * l.LD + i] = 0.0f; }
+    const int LD = l.LD;
     int* ibs = reinterpret_cast<int*>(sm + l.ibs);
     const int am = tid % TM, rg = tid / TM;
     const int ib = a.b.alist[(size_t)tile * TM + am];
-    if (rg == 0) ibs[am] = ib;
-    const int LD = l.LD;
-    __syncthreads();
-    {   // gather
+    {   // per-atom inputs of the tile, straight into shared memory
         const float *qp = nullptr, *qdp = nullptr, *fpp = nullptr, *Bp = nullptr, *Bdp = nullptr;
         float epsi = 0.0f;
         if (ib >= 0) {
@@ -345,29 +365,38 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
             Bp = sb_ptr(a.d.B, bi.x, l.TK, ln); Bdp = sb_ptr(a.b.Bd, w, l.TK, ln);
             if (rg == 0) epsi = a.b.eps[bi.y];
         }
-        gather_rows<true>(sm + l.Qs + am, LD, qp, 0, m.D, rg, RG, sm + l.sc);
-        gather_rows<true>(sm + l.QDs + am, LD, qdp, m.nR, m.D, rg, RG, sm + l.sc);
-        gather_rows<false>(sm + l.FPs + am, LD, fpp, 0, m.nR, rg, RG, nullptr);
-        gather_rows<false>(sm + l.Bs + am, LD, Bp, 0, l.TK, rg, RG, nullptr);
-        gather_rows<false>(sm + l.BDs + am, LD, Bdp, 0, l.TK, rg, RG, nullptr);
-        if (rg == 0) sm[l.aux + am] = epsi;
+        gather_rows(sm + l.BDs + am, LD, Bdp, 0, l.TK, rg, RG);
+        gather_rows(sm + l.QDs + am, LD, qdp, m.nR, m.D, rg, RG);
+        gather_rows(sm + l.Qs + am, LD, qp, 0, m.D, rg, RG);
+        gather_rows(sm + l.FPs + am, LD, fpp, 0, m.nR, rg, RG);
+        gather_rows(sm + l.Bs + am, LD, Bp, 0, l.TK, rg, RG);
+        cp_async_commit();
+        if (rg == 0) { sm[l.aux + am] = epsi; ibs[am] = ib; }
         for (int v = m.D + rg; v < l.DP8; v += RG) { sm[l.Qs + v * LD + am] = 0.0f; sm[l.QDs + v * LD + am] = 0.0f; }
     }
+    const int t = tile_type(a.b, tile, m.T);
+    ann_load_weights(a, l, sm, t, false);
+    for (int i = tid; i < l.TK * l.nR8; i += NT) {   // cRt[(tj, k)][n]
+        const int r = i / l.nR8, n = i - r * l.nR8, tj = r / m.KR, k = r - tj * m.KR;
+        sm[l.cRt + i] = (n < m.nR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
+    }
+    for (int i = tid; i < (l.HP32 - l.HP8) * l.LD; i += NT) { sm[l.Gs + l.HP8 * l.LD + i] = 0.0f; sm[l.Es + l.HP8 * l.LD + i] = 0.0f; }
+    cp_async_wait<0>();
     __syncthreads();
     const int ty = tid >> 3, tx = tid & 7, m0 = ty * AT;
-    // radial tangent: qd_n = sum_{T', k} cR[t][T'][n][k] Bd_k[T'], scaled
-    for_chunks(l.nR8 / 8, [&](int j0, auto cwc) {
+    // radial tangent: qd_n = sum_{T', k} cR[t][T'][n][k] Bd_k[T']
+    for_outputs(l.nR8, tx, [&](int o0, int ostep, auto cwc, auto quadc) {
         constexpr int CW = decltype(cwc)::value;
+        constexpr bool QUAD = decltype(quadc)::value;
         float acc[AT][CW];
-        tile_gemm<AT, CW>(sm + l.BDs + m0, LD, sm + l.cRt + tx + 8 * j0, l.nR8, 8, l.TK, acc);
+        tile_gemm<AT, CW, QUAD>(sm + l.BDs + m0, LD, sm + l.cRt + o0, l.nR8, ostep, l.TK, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
-            const int n = tx + 8 * (j0 + j);
+            const int n = o0 + j * ostep;
             if (n < m.nR) {
-                const float s = sm[l.sc + n];
                 float o[AT];
 #pragma unroll
-                for (int i = 0; i < AT; ++i) o[i] = s * acc[i][j];
+                for (int i = 0; i < AT; ++i) o[i] = acc[i][j];
                 store_atoms<AT>(sm + l.QDs + n * LD + m0, o);
             }
         }
@@ -380,26 +409,29 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
     bool valid[AT];
 #pragma unroll
     for (int i = 0; i < AT; ++i) valid[i] = ibs[m0 + i] >= 0;
-    for_chunks(l.NH, [&](int j0, auto cwc) {
+    for_outputs(l.HP8, tx, [&](int o0, int ostep, auto cwc, auto quadc) {
         constexpr int CW = decltype(cwc)::value;
+        constexpr bool QUAD = decltype(quadc)::value;
+        float hh[CW][AT];
+#pragma unroll
+        for (int j = 0; j < CW; ++j) load_atoms<AT>(hb + (size_t)(o0 + j * ostep) * TM + m0, hh[j]);   // in flight during the GEMM
         float acc[AT][CW];
-        tile_gemm<AT, CW>(sm + l.QDs + m0, LD, sm + l.W0m + (tx + 8 * j0) * l.DPs, 1, 8 * l.DPs, m.D, acc);
+        tile_gemm<AT, CW, QUAD>(sm + l.QDs + m0, LD, sm + l.W0t + o0, l.HP8, ostep, m.D, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
-            const int mu = tx + 8 * (j0 + j);
+            const int mu = o0 + j * ostep;
             const float w1 = sm[l.w1 + mu];
-            float h[AT];
-            load_atoms<AT>(hb + (size_t)mu * TM + m0, h);
             float gam[AT], e[AT], sg = 0.0f, sw = 0.0f;
 #pragma unroll
             for (int i = 0; i < AT; ++i) {
-                const float omh2 = fmaf(-h[i], h[i], 1.0f);
+                const float h = hh[j][i];
+                const float omh2 = fmaf(-h, h, 1.0f);
                 const float ee = valid[i] ? w1 * omh2 : 0.0f;
                 const float xd = acc[i][j];
                 e[i] = ee;
-                gam[i] = fmaf(epsv[i], ee, -2.0f * h[i] * ee * xd);
+                gam[i] = fmaf(epsv[i], ee, -2.0f * h * ee * xd);
                 sg += gam[i];
-                sw += valid[i] ? fmaf(epsv[i], h[i], omh2 * xd) : 0.0f;
+                sw += valid[i] ? fmaf(epsv[i], h, omh2 * xd) : 0.0f;
             }
             store_atoms<AT>(sm + l.Gs + mu * LD + m0, gam);
             store_atoms<AT>(sm + l.Es + mu * LD + m0, e);
@@ -423,15 +455,15 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
             atomicAdd(gt + which * m.H + mu, which ? s : -s);
         }
     }
-    {   // g_w0[t][mu][v] += sum_atoms gamma_mu q~_v + e_mu (s qd)_v : thread = rows {ra + RS jr} x cols {cb + 8 jc}
+    {   // g_w0[t][mu][v] += s_v sum_atoms (gamma_mu q_v + e_mu qd_v) : thread = rows {ra + RS jr} x cols {cb + 8 jc}
         constexpr int RS = NT / 8;
         const int ra = tid >> 3, cb = tid & 7;
         float* gt = a.g + (size_t)t * m.per_type;
-        const int nrg = (l.HP8 + RS - 1) / RS;          // row groups that hold real rows (rows up to HP16 are zero)
+        const int nrg = (l.HP8 + RS - 1) / RS;          // row groups that hold real rows (rows up to HP32 are zero)
         for (int jr0 = 0; jr0 < nrg; jr0 += 2) {
             const bool two = jr0 + 1 < nrg;
             const int r0 = ra + RS * jr0;
-            for_chunks(l.NV, [&](int jc0, auto cwc) {
+            for_chunks(l.DP8 / 8, [&](int jc0, auto cwc) {
                 constexpr int CW = decltype(cwc)::value;
                 const int c0 = cb + 8 * jc0;
                 if (two) {
@@ -442,7 +474,7 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
 #pragma unroll
                         for (int cc = 0; cc < CW; ++cc) {
                             const int mu = r0 + RS * r, v = c0 + 8 * cc;
-                            if (mu < m.H && v < m.D) atomicAdd(gt + mu * m.D + v, acc[r][cc]);
+                            if (mu < m.H && v < m.D) atomicAdd(gt + mu * m.D + v, sm[l.sc + v] * acc[r][cc]);
                         }
                 } else {
                     float acc[1][CW];
@@ -450,26 +482,25 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
 #pragma unroll
                     for (int cc = 0; cc < CW; ++cc) {
                         const int v = c0 + 8 * cc;
-                        if (r0 < m.H && v < m.D) atomicAdd(gt + r0 * m.D + v, acc[0][cc]);
+                        if (r0 < m.H && v < m.D) atomicAdd(gt + r0 * m.D + v, sm[l.sc + v] * acc[0][cc]);
                     }
                 }
             });
         }
     }
     __syncthreads();
-    // Qb = s o (w0^T gamma), written over q~
-    for_chunks(l.NV, [&](int j0, auto cwc) {
+    // Qb = s o (w0^T gamma), written over q
+    for_outputs(l.DP8, tx, [&](int o0, int ostep, auto cwc, auto quadc) {
         constexpr int CW = decltype(cwc)::value;
+        constexpr bool QUAD = decltype(quadc)::value;
         float acc[AT][CW];
-        tile_gemm<AT, CW>(sm + l.Gs + m0, LD, sm + l.W0m + tx + 8 * j0, l.DPs, 8, m.H, acc);
+        tile_gemm<AT, CW, QUAD>(sm + l.Gs + m0, LD, sm + l.W0m + o0, l.DP8, ostep, m.H, acc);
 #pragma unroll
         for (int j = 0; j < CW; ++j) {
-            const int v = tx + 8 * (j0 + j);
-            const float s = sm[l.sc + v];
             float o[AT];
 #pragma unroll
-            for (int i = 0; i < AT; ++i) o[i] = s * acc[i][j];
-            store_atoms<AT>(sm + l.Qs + v * LD + m0, o);
+            for (int i = 0; i < AT; ++i) o[i] = acc[i][j];
+            store_atoms<AT>(sm + l.Qs + (o0 + j * ostep) * LD + m0, o);
         }
     });
     __syncthreads();
