@@ -74,6 +74,45 @@ static int upload(nep_ctx* c, T*& dptr, const T* h, size_t count)
     return NEP_OK;
 }
 
+namespace nep {
+// Per-slot tables of the current slot order (h_slot_of): species and rank among the same species per slot, the atom of
+// every slot and the slot of every atom; the force labels follow if they are loaded.
+int upload_slot_tables(nep_ctx* c)
+{
+    DataDev& d = c->d;
+    const int T = c->m.T;
+    std::vector<int> type_p((size_t)c->NP, -1), rank_p((size_t)c->NP, 0), orig_p((size_t)c->NP, -1);
+    for (int s = 0; s < c->S; ++s) {
+        const int64_t a0 = c->h_aoff[s], p0 = c->h_pbase[s];
+        for (int i = 0; i < c->h_nat[s]; ++i) { const int sl = c->h_slot_of[a0 + i]; orig_p[p0 + sl] = i; type_p[p0 + sl] = c->h_type[a0 + i]; }
+        std::vector<int> tc(T, 0);
+        for (int sl = 0; sl < c->h_nat[s]; ++sl) rank_p[p0 + sl] = tc[type_p[p0 + sl]]++;
+    }
+    const void* olds[] = { d.type_p, d.rank_p, d.orig_p, d.slot_of };
+    for (const void* p : olds) dev_free(c, const_cast<void*>(p));
+    d.type_p = d.rank_p = d.orig_p = d.slot_of = nullptr;
+    int *dtp, *drk, *dor, *dso;
+    int rc;
+    if ((rc = upload<int>(c, dtp, type_p.data(), type_p.size()))) return rc;
+    if ((rc = upload<int>(c, drk, rank_p.data(), rank_p.size()))) return rc;
+    if ((rc = upload<int>(c, dor, orig_p.data(), orig_p.size()))) return rc;
+    if ((rc = upload<int>(c, dso, c->h_slot_of.data(), c->h_slot_of.size()))) return rc;
+    d.type_p = dtp; d.rank_p = drk; d.orig_p = dor; d.slot_of = dso;
+    if (c->have_labels && !c->h_Flab.empty()) {
+        std::vector<float> Fp((size_t)3 * c->NP, 0.0f);
+        for (int s = 0; s < c->S; ++s)
+            for (int i = 0; i < c->h_nat[s]; ++i)
+                for (int k = 0; k < 3; ++k) {
+                    const int64_t p = c->h_pbase[s] + c->h_slot_of[c->h_aoff[s] + i];
+                    Fp[(size_t)((p / WARP) * 3 + k) * WARP + p % WARP] = c->h_Flab[3 * (c->h_aoff[s] + i) + k];
+                }
+        NEP_CUDA(c, cudaMemcpyAsync(const_cast<float*>(d.Flab), Fp.data(), 4 * Fp.size(), cudaMemcpyHostToDevice, c->stream));
+    }
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NEP_OK;
+}
+}  // namespace nep
+
 extern "C" {
 
 const char* nep_version(void) { return "nep_b200 0.2 (sm_100a, fp32 step, fp64 neighbour predicate)"; }
@@ -152,7 +191,7 @@ int64_t nep_num_params(const nep_ctx* c) { return c ? c->m.npar : NEP_EINVAL; }
 static void free_dataset(nep_ctx* c)
 {
     DataDev& d = c->d;
-    const void* ptrs[] = { d.pos, d.box, d.type, d.atom_off, d.pbase, d.type_p, d.rank_p, d.slice_struct, d.Elab, d.Flab, d.Wlab, d.hasv,
+    const void* ptrs[] = { d.pos, d.box, d.type, d.atom_off, d.pbase, d.type_p, d.rank_p, d.orig_p, d.slot_of, d.slice_struct, d.Elab, d.Flab, d.Wlab, d.hasv,
                            d.offR, d.jR, d.shR, d.offA, d.jA, d.shA, d.cntR, d.recoffR, d.recR, d.cntA, d.recoffA, d.recA, d.B };
     for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
     memset(&d, 0, sizeof d);
@@ -168,11 +207,13 @@ static int upload_labels(nep_ctx* c, const double* E, const double* F, const dou
     for (int64_t i = 0; i < 3 * c->N; ++i) if (!std::isfinite(F[i])) return fail(c, NEP_EINVAL, "non-finite force label");
     for (int64_t i = 0; i < 9 * (int64_t)c->S; ++i) if (!std::isfinite(W[i])) return fail(c, NEP_EINVAL, "non-finite virial label");
     std::vector<float> Fp((size_t)3 * c->NP, 0.0f), Wf((size_t)9 * c->S);
+    c->h_Flab.resize((size_t)3 * c->N);
+    for (int64_t i = 0; i < 3 * c->N; ++i) c->h_Flab[i] = (float)F[i];
     for (int s = 0; s < c->S; ++s)
         for (int i = 0; i < c->h_nat[s]; ++i)
-            for (int k = 0; k < 3; ++k) {   // slice-blocked [slice][3][32]
-                const int64_t p = c->h_pbase[s] + i;
-                Fp[(size_t)((p / WARP) * 3 + k) * WARP + p % WARP] = (float)F[3 * (c->h_aoff[s] + i) + k];
+            for (int k = 0; k < 3; ++k) {   // slice-blocked [slice][3][32], slot order
+                const int64_t p = c->h_pbase[s] + c->h_slot_of[c->h_aoff[s] + i];
+                Fp[(size_t)((p / WARP) * 3 + k) * WARP + p % WARP] = c->h_Flab[3 * (c->h_aoff[s] + i) + k];
             }
     for (size_t i = 0; i < Wf.size(); ++i) Wf[i] = (float)W[i];
     c->h_hasv.assign(c->S, 1);
@@ -228,31 +269,28 @@ int nep_load_structures(nep_ctx* c, int S, const int* n_atoms, const double* pos
     free_dataset(c);
     c->S = S; c->N = N; c->NP = NP; c->nslices = (int)(NP / WARP);
     c->h_nat.assign(n_atoms, n_atoms + S); c->h_aoff = aoff; c->h_pbase = pbase; c->h_box.assign(box, box + 9 * (size_t)S);
-    std::vector<int> type_p((size_t)NP, -1), rank_p((size_t)NP, 0), slice_struct((size_t)c->nslices, 0);
+    std::vector<int> slice_struct((size_t)c->nslices, 0);
     c->h_tcount.assign((size_t)S * c->m.T, 0);
+    c->h_type.assign(type, type + N);
+    c->h_slot_of.resize((size_t)N);
+    c->h_Flab.clear();
     for (int s = 0; s < S; ++s) {
-        int* tc = &c->h_tcount[(size_t)s * c->m.T];
-        for (int i = 0; i < n_atoms[s]; ++i) {
-            const int t = type[aoff[s] + i];
-            type_p[pbase[s] + i] = t;
-            rank_p[pbase[s] + i] = tc[t]++;
-        }
+        for (int i = 0; i < n_atoms[s]; ++i) { c->h_slot_of[aoff[s] + i] = i; c->h_tcount[(size_t)s * c->m.T + type[aoff[s] + i]]++; }
         for (int64_t sl = pbase[s] / WARP; sl < pbase[s + 1] / WARP; ++sl) slice_struct[sl] = s;
     }
     DataDev& d = c->d;
     d.S = S; d.N = N; d.NP = NP; d.nslices = c->nslices;
     int rc;
-    double *dpos, *dbox; int *dtype, *dtp, *drk, *dss; int64_t *dao, *dpb;
+    double *dpos, *dbox; int *dtype, *dss; int64_t *dao, *dpb;
     if ((rc = upload<double>(c, dpos, pos, 3 * (size_t)N))) return rc;
     if ((rc = upload<double>(c, dbox, box, 9 * (size_t)S))) return rc;
     if ((rc = upload<int>(c, dtype, type, (size_t)N))) return rc;
-    if ((rc = upload<int>(c, dtp, type_p.data(), type_p.size()))) return rc;
-    if ((rc = upload<int>(c, drk, rank_p.data(), rank_p.size()))) return rc;
     if ((rc = upload<int>(c, dss, slice_struct.data(), slice_struct.size()))) return rc;
     if ((rc = upload<int64_t>(c, dao, aoff.data(), aoff.size()))) return rc;
     if ((rc = upload<int64_t>(c, dpb, pbase.data(), pbase.size()))) return rc;
     NEP_CUDA(c, cudaStreamSynchronize(c->stream));
-    d.pos = dpos; d.box = dbox; d.type = dtype; d.type_p = dtp; d.rank_p = drk; d.slice_struct = dss; d.atom_off = dao; d.pbase = dpb;
+    d.pos = dpos; d.box = dbox; d.type = dtype; d.slice_struct = dss; d.atom_off = dao; d.pbase = dpb;
+    if ((rc = upload_slot_tables(c))) return rc;
     c->have_data = true;
     if (lab) return upload_labels(c, E, F, W, has_virial);
     c->h_hasv.assign(S, 1);

@@ -42,6 +42,8 @@ struct DataDev {
     const int64_t* atom_off;   // [S+1]
     const int64_t* pbase;      // [S+1] padded offset of each structure
     const int* type_p;     // [NP], -1 = padding
+    const int* orig_p;     // [NP] structure-local index (caller's order) of the atom in this slot, -1 = padding
+    const int* slot_of;    // [N]  structure-local slot of every atom: the inverse of orig_p
     const int* rank_p;     // [NP] rank of the atom among the atoms of its own type in its structure
     const int* slice_struct;   // [nslices]
     // labels
@@ -122,6 +124,10 @@ struct nep_ctx {
     std::vector<int> h_nat; std::vector<int64_t> h_aoff, h_pbase; std::vector<unsigned char> h_hasv;
     std::vector<int> h_tcount;   // [S][T] atoms of each type
     std::vector<double> h_box;
+    // Slot order inside a structure: atoms sorted by (species, angular neighbour count) so that the
+    // 32 lanes of a slice share a species and walk pair lists of similar length.  Identity until the lists exist.
+    std::vector<int> h_type, h_slot_of;   // [N] species ; structure-local slot of every atom
+    std::vector<float> h_Flab;            // [N][3] force labels in the caller's order (re-laid out when the slot order changes)
     bool have_data = false, have_labels = false, have_nbrs = false, have_params = false, have_scaler = false;
     bool forward_valid = false, grad_valid = false;
     int64_t PR = 0, PA = 0;
@@ -160,6 +166,7 @@ void prof_end(nep_ctx* c);
     } while (0)
 
 // ---- launchers (each returns NEP_OK or an error code with c->err set) ----
+int upload_slot_tables(nep_ctx* c);                            // nep_api.cu      : type_p, rank_p, orig_p, slot_of, force labels from h_slot_of
 int build_neighbors_dev(nep_ctx* c);                           // nep_neighbor.cu : S0a + S0b
 int launch_forward(nep_ctx* c, bool descriptors_only);         // nep_step.cu     : S1-S5
 int launch_loss_grad(nep_ctx* c);                              // nep_step.cu     : S6-S9

@@ -124,8 +124,9 @@ __global__ void k_gather_outputs(StepArgs a, float* E, float* F, float* W)
     if (F && i < a.b.NBP) {
         const int w = (int)(i >> 5), lane = (int)(i & 31);
         const int4 bi = a.b.binfo[w];
-        if (a.d.type_p[(size_t)bi.x * WARP + lane] >= 0) {
-            const int64_t o = a.b.bfoff[bi.y] + (i - bi.z);
+        const int il = a.d.orig_p[(size_t)bi.x * WARP + lane];
+        if (il >= 0) {
+            const int64_t o = a.b.bfoff[bi.y] + il;
             const float* Fp = sb_ptr(a.b.F, w, 3, lane);
             F[3 * o] = Fp[0]; F[3 * o + 1] = Fp[WARP]; F[3 * o + 2] = Fp[2 * WARP];
         }
@@ -137,8 +138,9 @@ __global__ void k_gather_q(StepArgs a, float* q)
     if (i >= a.b.NBP) return;
     const int w = (int)(i >> 5), lane = (int)(i & 31);
     const int4 bi = a.b.binfo[w];
-    if (a.d.type_p[(size_t)bi.x * WARP + lane] < 0) return;
-    const int64_t o = a.b.bfoff[bi.y] + (i - bi.z);
+    const int il = a.d.orig_p[(size_t)bi.x * WARP + lane];
+    if (il < 0) return;
+    const int64_t o = a.b.bfoff[bi.y] + il;
     const float* qp = sb_ptr(a.b.q, w, a.m.D, lane);
     for (int v = 0; v < a.m.D; ++v) q[o * a.m.D + v] = qp[(size_t)v * WARP];
 }

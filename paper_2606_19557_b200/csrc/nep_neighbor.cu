@@ -187,7 +187,7 @@ __global__ void k_nbr_sort(int64_t N, const unsigned long long* __restrict__ key
 
 // per padded atom: neighbour counts (0 for padding); per slice: width = max count
 __global__ void k_slice_width(int nslices, const int64_t* __restrict__ pbase, const int64_t* __restrict__ atom_off,
-                              const int* __restrict__ slice_struct, const int* __restrict__ type_p,
+                              const int* __restrict__ slice_struct, const int* __restrict__ orig_p,
                               const int64_t* __restrict__ off, int* __restrict__ cnt_p, int* __restrict__ width)
 {
     int sl = (blockIdx.x * blockDim.x + threadIdx.x) / WARP, lane = threadIdx.x & 31;
@@ -195,8 +195,8 @@ __global__ void k_slice_width(int nslices, const int64_t* __restrict__ pbase, co
     int64_t ip = (int64_t)sl * WARP + lane;
     int s = slice_struct[sl];
     int c = 0;
-    if (type_p[ip] >= 0) {
-        int64_t ig = atom_off[s] + (ip - pbase[s]);
+    if (orig_p[ip] >= 0) {
+        int64_t ig = atom_off[s] + orig_p[ip];
         c = (int)(off[ig + 1] - off[ig]);
     }
     cnt_p[ip] = c;
@@ -222,20 +222,20 @@ __device__ void basis_f64(double r, double rc, int K, double* f)
 template <bool RADIAL>
 __global__ void k_cache_fill(int nslices, ModelDev m, const double* __restrict__ pos, const double* __restrict__ box,
                              const int* __restrict__ type, const int64_t* __restrict__ pbase, const int64_t* __restrict__ atom_off,
-                             const int* __restrict__ slice_struct, const int* __restrict__ type_p,
+                             const int* __restrict__ slice_struct, const int* __restrict__ orig_p, const int* __restrict__ slot_of,
                              const int64_t* __restrict__ off, const int* __restrict__ nj, const signed char* __restrict__ sh,
                              const int64_t* __restrict__ recoff, float4* __restrict__ rec, float* __restrict__ B, int64_t NP)
 {
     int sl = (blockIdx.x * blockDim.x + threadIdx.x) / WARP, lane = threadIdx.x & 31;
     if (sl >= nslices) return;
     int64_t ip = (int64_t)sl * WARP + lane;
-    if (type_p[ip] < 0) {
+    if (orig_p[ip] < 0) {
         if (RADIAL) for (int k = 0; k < m.T * m.KR; ++k) B[((int64_t)sl * m.T * m.KR + k) * WARP + lane] = 0.0f;
         return;
     }
     int s = slice_struct[sl];
     int64_t a0 = atom_off[s];
-    int il = (int)(ip - pbase[s]);
+    int il = orig_p[ip];
     int64_t ig = a0 + il;
     double bx[9], ri[3];
     for (int k = 0; k < 9; ++k) bx[k] = box[9 * (int64_t)s + k];
@@ -251,7 +251,7 @@ __global__ void k_cache_fill(int nslices, ModelDev m, const double* __restrict__
             if (type[a0 + jl] != t) continue;
             double rj[3] = { pos[3 * (a0 + jl)], pos[3 * (a0 + jl) + 1], pos[3 * (a0 + jl) + 2] }, d[3];
             bond_rn(ri, rj, bx, sh[3 * p], sh[3 * p + 1], sh[3 * p + 2], d);
-            out[(int64_t)slot * WARP] = make_float4((float)d[0], (float)d[1], (float)d[2], __int_as_float(jl | (t << 24)));
+            out[(int64_t)slot * WARP] = make_float4((float)d[0], (float)d[1], (float)d[2], __int_as_float(slot_of[a0 + jl] | (t << 24)));
             ++slot;
             if (RADIAL) {
                 double f[17];
@@ -362,6 +362,25 @@ int build_neighbors_dev(nep_ctx* c)
         c->h_pairsR_struct[s] = hoR[c->h_aoff[s + 1]] - hoR[c->h_aoff[s]];
         c->h_pairsA_struct[s] = hoA[c->h_aoff[s + 1]] - hoA[c->h_aoff[s]];
     }
+    // slot order inside every structure: (species, angular neighbour count descending, caller's index)
+    {
+        std::vector<int> order;
+        for (int s = 0; s < S; ++s) {
+            const int64_t a0 = c->h_aoff[s];
+            const int n = c->h_nat[s];
+            order.resize(n);
+            for (int i = 0; i < n; ++i) order[i] = i;
+            std::sort(order.begin(), order.end(), [&](int x, int y) {
+                const int tx = c->h_type[a0 + x], ty = c->h_type[a0 + y];
+                if (tx != ty) return tx < ty;
+                const int64_t cx = hoA[a0 + x + 1] - hoA[a0 + x], cy = hoA[a0 + y + 1] - hoA[a0 + y];
+                if (cx != cy) return cx > cy;
+                return x < y;
+            });
+            for (int sl = 0; sl < n; ++sl) c->h_slot_of[a0 + order[sl]] = sl;
+        }
+        if ((rc = upload_slot_tables(c))) return rc;
+    }
     DALLOC(keys, unsigned long long, PR);
     DALLOC(jR, int, PR); DALLOC(shR, signed char, 3 * PR); DALLOC(jA, int, PA); DALLOC(shA, signed char, 3 * PA);
     prof_begin(c, "k_nbr_fill");
@@ -381,10 +400,10 @@ int build_neighbors_dev(nep_ctx* c)
     DALLOC(cntRp, int, c->NP); DALLOC(cntAp, int, c->NP); DALLOC(wR, int, ns); DALLOC(wA, int, ns);
     DALLOC(recoffR, int64_t, ns + 1); DALLOC(recoffA, int64_t, ns + 1);
     prof_begin(c, "k_slice_width");
-    k_slice_width<<<gS, TB, 0, c->stream>>>(ns, d.pbase, d.atom_off, d.slice_struct, d.type_p, offR, cntRp, wR);
+    k_slice_width<<<gS, TB, 0, c->stream>>>(ns, d.pbase, d.atom_off, d.slice_struct, d.orig_p, offR, cntRp, wR);
     prof_end(c);
     prof_begin(c, "k_slice_width");
-    k_slice_width<<<gS, TB, 0, c->stream>>>(ns, d.pbase, d.atom_off, d.slice_struct, d.type_p, offA, cntAp, wA);
+    k_slice_width<<<gS, TB, 0, c->stream>>>(ns, d.pbase, d.atom_off, d.slice_struct, d.orig_p, offA, cntAp, wA);
     prof_end(c);
     if ((rc = scan_excl(c, wR, recoffR, ns, WARP))) return rc;
     if ((rc = scan_excl(c, wA, recoffA, ns, WARP))) return rc;
@@ -396,11 +415,11 @@ int build_neighbors_dev(nep_ctx* c)
     NEP_CUDA(c, cudaMemsetAsync(recR, 0, 16 * (size_t)std::max<int64_t>(totR, 1), c->stream));
     NEP_CUDA(c, cudaMemsetAsync(recA, 0, 16 * (size_t)std::max<int64_t>(totA, 1), c->stream));
     prof_begin(c, "k_cache_fill_R");
-    k_cache_fill<true><<<gS, TB, 0, c->stream>>>(ns, m, d.pos, d.box, d.type, d.pbase, d.atom_off, d.slice_struct, d.type_p,
+    k_cache_fill<true><<<gS, TB, 0, c->stream>>>(ns, m, d.pos, d.box, d.type, d.pbase, d.atom_off, d.slice_struct, d.orig_p, d.slot_of,
                                                 offR, jR, shR, recoffR, recR, B, c->NP);
     prof_end(c);
     prof_begin(c, "k_cache_fill_A");
-    k_cache_fill<false><<<gS, TB, 0, c->stream>>>(ns, m, d.pos, d.box, d.type, d.pbase, d.atom_off, d.slice_struct, d.type_p,
+    k_cache_fill<false><<<gS, TB, 0, c->stream>>>(ns, m, d.pos, d.box, d.type, d.pbase, d.atom_off, d.slice_struct, d.orig_p, d.slot_of,
                                                  offA, jA, shA, recoffA, recA, nullptr, c->NP);
     prof_end(c);
     NEP_CUDA(c, cudaGetLastError());
