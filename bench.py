@@ -144,9 +144,28 @@ def setup_ours(w, stream=None):
     return nep, dict(load_s=t1 - t0, neighbors_cache_s=t2 - t1, params_labels_s=time.time() - t2)
 
 
+DP = {"world": 1, "views": None}   # data-parallel state of this process (world > 1: every rank holds one copy of the
+                                    # config's structures as its share of a `world` times larger set and batch)
+
+
+def dp_whole_batch(nep):
+    """Eqs. 5-7 divide by the counts of the WHOLE batch = world x this rank's (every rank runs the same shapes)."""
+    if DP["world"] > 1 or DP["views"] is not None:
+        Sb, Nb = nep.batch_shape()
+        nep.set_batch_normalisers(DP["world"] * Sb, DP["world"] * Nb, DP["world"] * Sb)
+
+
+def dp_exchange(nep):
+    """The step's one exchange (paper_2606_19557_b200/dataparallel.py): NCCL all-reduce of g and of the 4 loss terms."""
+    if DP["views"] is not None:
+        from paper_2606_19557_b200.dataparallel import allreduce_grad_loss
+        allreduce_grad_loss(*DP["views"])
+
+
 def one_step(nep, lam):
     nep.forward_device()
     nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
+    dp_exchange(nep)
     nep.adam_step(LR)
 
 
@@ -154,8 +173,14 @@ def e2e_step(nep, lam, ids):
     """The call sequence a user makes per training step, HOST buffers in and out: the batch's structure ids go in
     (nep_set_batch copies them and the slice tables to the device), the loss comes back (nep_loss_grad -> host)."""
     nep.set_batch(ids)
+    dp_whole_batch(nep)
     nep.forward_device()
-    l4 = nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=True)
+    if DP["views"] is None:
+        l4 = nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=True)
+    else:
+        nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
+        dp_exchange(nep)
+        l4 = DP["views"][1].cpu().numpy()          # the whole batch's loss terms -> host
     nep.adam_step(LR)
     return l4
 
@@ -168,17 +193,27 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the NEP step has no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    use_dist = world > 1 or os.environ.get("NEP_BENCH_DIST") == "1"    # NEP_BENCH_DIST=1: run the NCCL path on one rank too
+    saved_stdout = None
+    if use_dist:
+        # NCCL prints its version banner on stdout; the contract is ONE JSON line there: park stdout on stderr until the end
+        sys.stdout.flush()
+        saved_stdout = os.dup(1)
+        os.dup2(2, 1)
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
     from paper_2606_19557_b200 import workloads as wl, roofline as rf
     from paper_2606_19557_b200 import build as nbuild
     if rank == 0:
         nbuild.build()
-    if world > 1:
+    if use_dist:
         dist.barrier()
     w = make_workload(args, rank)
     nep, setup = setup_ours(w)
     lam = w.lambdas
+    DP["world"] = world
+    if use_dist:
+        DP["views"] = nep.grad_loss_tensors()
     blist = wl.batches(w)
     full_batches = [b for b in blist if len(b) == w.batch_size] or blist
     single = len(blist) == 1
@@ -191,10 +226,12 @@ def run_ours(args):
     def set_b(i):
         if not single:
             nep.set_batch(full_batches[i % len(full_batches)])
+            dp_whole_batch(nep)
 
     # ---- warm-up ----
     if single:
         nep.set_batch(None)
+        dp_whole_batch(nep)
     for i in range(max(args.warmup, 3)):
         set_b(i); one_step(nep, lam)
     torch.cuda.synchronize()
@@ -278,8 +315,7 @@ def run_ours(args):
     e2e_value = e_atoms / (e2e_ms * 1e-3)
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        dist.destroy_process_group()
         return
     # ---- roofline of the dominant kernel ----
     if single:
@@ -319,7 +355,8 @@ def run_ours(args):
                    "atoms_per_step": atoms // K // world, "pairs_R_per_step": sizes["P_R_b"], "pairs_A_per_step": sizes["P_A_b"],
                    "l2": ("flushed between timed steps (256 MB write)" if flush is not None else "not flushed; per-step working set exceeds L2"),
                    "ms_per_step_back_to_back_no_flush": ms_b2b, "setup_s": setup,
-                   "device_bytes": nep.bytes_allocated, "parallelism": f"dp{world} (structures sharded, no data-path collective)"},
+                   "device_bytes": nep.bytes_allocated, "parallelism": (f"dp{world}: structures sharded, whole batch = {world} x {w.batch_size} structures, one NCCL all-reduce of g "
+                                    f"[{w.model.n_par} fp32] + 4 loss terms per step" if use_dist else "dp1 (one GPU, no collective)")},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
                 "what": "per step: nep_set_batch(host ids) + nep_forward + nep_loss_grad(loss -> host) + nep_adam_step; geometry cache resident (P:143)"},
         "gpu_launches": int(launches),
@@ -333,8 +370,11 @@ def run_ours(args):
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(args, w, seconds_target=15.0)
     nep.destroy()
-    print(json.dumps(out))
-    if world > 1:
+    if saved_stdout is not None:
+        sys.stdout.flush()
+        os.dup2(saved_stdout, 1)
+    print(json.dumps(out), flush=True)
+    if use_dist:
         dist.destroy_process_group()
 
 

@@ -139,6 +139,18 @@ int nep_get_descriptors(nep_ctx* ctx, float* q);
 int nep_loss_grad(nep_ctx* ctx, double lambda_E, double lambda_F, double lambda_V, double* loss4_host);
 int nep_get_loss(nep_ctx* ctx, double* loss4_host);
 
+/* Data-parallel training over several contexts, one per GPU.  Structures interact only with
+ * themselves (Eq. 1), so the batch of a step is split by structure: every context holds its share of the data
+ * set and calls nep_set_batch with its share of the batch.  The loss of Eq. 4 and its gradient (Eq. 8) are sums over
+ * structures and atoms divided by the batch counts of Eqs. 5-7, so with the counts of the WHOLE batch given here
+ * (S_b structures, N_b atoms, S_v structures with virial labels; each >= this context's own count, NEP_EINVAL otherwise)
+ * every context produces its additive share of {L, dE, dF, dV} and of g.  The caller sums g [N_par floats] and the four
+ * loss terms [4 doubles] over the contexts in place -- device pointers from nep_grad_device_ptr, e.g. one NCCL
+ * all-reduce each -- and then calls nep_adam_step on every context (identical updates, no parameter broadcast).
+ * nep_set_batch resets the counts to those of the local batch.  Call after nep_set_batch, before nep_loss_grad. */
+int nep_set_batch_normalisers(nep_ctx* ctx, int64_t n_struct_whole, int64_t n_atoms_whole, int64_t n_virial_whole);
+int nep_grad_device_ptr(nep_ctx* ctx, float** g, double** loss4);
+
 /* S10: Adam with AMSGrad on theta with the stored gradient.  variant 0 = Eqs. 9-13 literally (running max of
  * the bias-corrected second moment, epsilon inside the root); variant 1 = torch.optim.Adam(amsgrad=True).
  * Increments the step count t.  Invalidates the forward results. */

@@ -50,6 +50,8 @@ SIGNATURES = {
     "nep_get_descriptors": (C.c_int, [_P, _P]),
     "nep_loss_grad": (C.c_int, [_P, C.c_double, C.c_double, C.c_double, _P]),
     "nep_get_loss": (C.c_int, [_P, _P]),
+    "nep_set_batch_normalisers": (C.c_int, [_P, C.c_int64, C.c_int64, C.c_int64]),
+    "nep_grad_device_ptr": (C.c_int, [_P, C.POINTER(_P), C.POINTER(_P)]),
     "nep_adam_step": (C.c_int, [_P, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int]),
     "nep_synchronize": (C.c_int, [_P]),
     "nep_launch_count": (C.c_int, [_P, C.POINTER(C.c_int64)]),
@@ -296,6 +298,26 @@ class Nep:
         l4 = np.zeros(4, np.float64)
         self._ck(self._L.nep_get_loss(self._h, _ptr(l4)))
         return l4
+
+    # ---- data-parallel training (include/nep.h: nep_set_batch_normalisers) ----
+    def set_batch_normalisers(self, n_struct_whole: int, n_atoms_whole: int, n_virial_whole: int):
+        self._ck(self._L.nep_set_batch_normalisers(self._h, int(n_struct_whole), int(n_atoms_whole), int(n_virial_whole)))
+
+    def grad_loss_tensors(self):
+        """(g, loss4): torch views (float32 [N_par], float64 [4]) of the context's gradient and loss terms on the device,
+        for in-place collectives.  Needs the torch allocator (the views alias the tensors it handed to the library)."""
+        g, l = C.c_void_p(None), C.c_void_p(None)
+        self._ck(self._L.nep_grad_device_ptr(self._h, C.byref(g), C.byref(l)))
+        torch = self._torch
+
+        def view(ptr, dtype, count):
+            isz = torch.empty(0, dtype=dtype).element_size()
+            for base, t in self._bufs.items():
+                if base <= ptr < base + t.numel():
+                    off = ptr - base
+                    return t[off:off + count * isz].view(dtype)
+            raise RuntimeError("device pointer is not inside a torch allocation (use_torch_allocator=False?)")
+        return view(g.value, torch.float32, self.n_par), view(l.value, torch.float64, 4)
 
     def adam_step(self, lr: float, beta1: float = 0.9, beta2: float = 0.999, eps: float = 1e-8, variant: int = 0):
         self._ck(self._L.nep_adam_step(self._h, lr, beta1, beta2, eps, variant))

@@ -306,7 +306,7 @@ int nep_set_labels(nep_ctx* c, const double* E, const double* F, const double* W
     if (rc == NEP_OK && c->have_nbrs) {   // Sv of the current batch depends on the mask
         int sv = 0;
         for (int sid : c->h_bsid) sv += c->h_hasv[sid];
-        c->b.Sv = sv;
+        c->b.Sv = sv; c->b.nrmV = (double)sv;
     }
     return rc;
 }
@@ -536,6 +536,7 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
         nbp += c->h_pbase[s + 1] - c->h_pbase[s];
     }
     b.Sb = Sb; b.Sv = Sv; b.Nb = Nb; b.nbs = nbs; b.NBP = nbp; b.tile_m = TM; b.ntiles = ntiles;
+    b.nrmS = (double)Sb; b.nrmN = (double)Nb; b.nrmV = (double)Sv;
     const size_t bytes = 16 * (size_t)nbs + 8 * (size_t)Sb + 4 * (size_t)Sb * (2 + T);
     char* d = (char*)c->d_stage;
     b.binfo = (const int4*)d;
@@ -598,6 +599,26 @@ int nep_get_descriptors(nep_ctx* c, float* q)
     if (!rc) rc = d2h(c, q, stage, 4 * n);
     dev_free(c, stage);
     return rc;
+}
+
+int nep_set_batch_normalisers(nep_ctx* c, int64_t n_struct, int64_t n_atoms, int64_t n_virial)
+{
+    CHECK_CTX(c);
+    if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_set_batch_normalisers before nep_build_neighbors");
+    if (n_struct < c->b.Sb || n_atoms < c->b.Nb || n_virial < c->b.Sv)
+        return fail(c, NEP_EINVAL, "the whole batch cannot be smaller than this context's share of it");
+    c->b.nrmS = (double)n_struct; c->b.nrmN = (double)n_atoms; c->b.nrmV = (double)n_virial;
+    c->grad_valid = false;
+    return NEP_OK;
+}
+
+int nep_grad_device_ptr(nep_ctx* c, float** g, double** loss4)
+{
+    CHECK_CTX(c);
+    if (!c->b.lacc) return fail(c, NEP_ESTATE, "nep_grad_device_ptr before nep_build_neighbors");
+    if (g) *g = c->g;
+    if (loss4) *loss4 = c->b.lacc + 4;
+    return NEP_OK;
 }
 
 int nep_get_loss(nep_ctx* c, double* loss4)

@@ -65,6 +65,7 @@ struct BatchDev {
     int Sb;                // structures in the batch
     int Sv;                // ... of which have virial labels
     int64_t Nb;            // atoms in the batch
+    double nrmS, nrmN, nrmV;   // normalisers of Eqs. 5-7: S_b, N_b, S_v of the WHOLE batch (= the local ones unless data-parallel)
     int nbs;               // slices in the batch
     int64_t NBP;           // nbs * 32
     const int4* binfo;     // [nbs] {data-set slice, batch structure index, batch-padded index of the structure's first atom, 0}

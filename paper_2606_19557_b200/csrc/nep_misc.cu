@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
         const int w = gid >> 5, lane = gid & 31;
         const int4 bi = __ldg(a.b.binfo + w);
         const bool valid = __ldg(a.d.type_p + (size_t)bi.x * WARP + lane) >= 0;
-        const float c = 2.0f * lamF / (3.0f * (float)a.b.Nb);
+        const float c = (float)(2.0 * dlamF / (3.0 * a.b.nrmN));
         const float* Fp = sb_ptr(a.b.F, w, 3, lane);
         const float* Fl = sb_ptr(a.d.Flab, bi.x, 3, lane);
         float* up = sb_ptr(a.b.u, w, 3, lane);
@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
         const double n = (double)a.b.bnat[sb];
         const double dE = a.b.Es[sb] - a.d.Elab[sid];
         sE = (dE / n) * (dE / n);                                                   // Eq. 5
-        const float eps = (float)(2.0 * dlamE * dE / ((double)a.b.Sb * n * n));
+        const float eps = (float)(2.0 * dlamE * dE / (a.b.nrmS * n * n));
         a.b.eps[sb] = eps;
         sB = (double)eps * n;
         const bool hv = a.d.hasv[sid] != 0;
@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
         for (int k = 0; k < 9; ++k) {
             const double t = hv ? (double)a.b.Ws[9 * sb + k] - (double)a.d.Wlab[9 * (size_t)sid + k] : 0.0;
             sW += (t / n) * (t / n);                                                // Eq. 7
-            a.b.G[9 * sb + k] = (hv && a.b.Sv > 0) ? (float)(2.0 * dlamV * t / (9.0 * a.b.Sv * n * n)) : 0.0f;
+            a.b.G[9 * sb + k] = (hv && a.b.nrmV > 0.0) ? (float)(2.0 * dlamV * t / (9.0 * a.b.nrmV * n * n)) : 0.0f;
         }
     }
     // block reduction -> one atomic per block and quantity
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
     if (last && threadIdx.x == 0) {
         __threadfence();
         volatile double* l = a.b.lacc;
-        const double dE = a.b.Sb ? l[0] / a.b.Sb : 0.0, dF = a.b.Nb ? l[1] / (3.0 * a.b.Nb) : 0.0, dV = a.b.Sv ? l[2] / (9.0 * a.b.Sv) : 0.0;
+        const double dE = a.b.nrmS > 0.0 ? l[0] / a.b.nrmS : 0.0, dF = a.b.nrmN > 0.0 ? l[1] / (3.0 * a.b.nrmN) : 0.0, dV = a.b.nrmV > 0.0 ? l[2] / (9.0 * a.b.nrmV) : 0.0;
         const double sb1 = l[3];
         l[4] = dlamE * dE + dlamF * dF + dlamV * dV; l[5] = dE; l[6] = dF; l[7] = dV;   // Eq. 4
         a.g[a.m.o_b1] = (float)(-sb1);                                                   // g_b1 = -sum_i eps_s(i)

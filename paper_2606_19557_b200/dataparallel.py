@@ -1,0 +1,138 @@
+"""Data-parallel NEP training over several GPUs, one process (rank) per GPU.
+
+Structures interact only with themselves (Eq. 1; the sums of Eqs. 15-20 run over the neighbours inside one
+periodic structure), so the units that shard are STRUCTURES:
+
+  * set-up   : every rank loads its own share of the data set (`shard_structures`: longest-processing-time partition
+               by pair-work estimate) and builds its own neighbour lists and pair cache; nothing is exchanged;
+  * per step : the batch (global structure ids) is cut by owner (`local_batch`); every rank runs nep_forward and
+               nep_loss_grad on its share with the batch counts of Eqs. 5-7 taken over the WHOLE batch
+               (nep_set_batch_normalisers), which makes its loss terms and its gradient additive shares;
+               ONE exchange: all-reduce (sum) of g [N_par fp32] and of {L, dE, dF, dV} [4 fp64]
+               (`allreduce_grad_loss`: NCCL on the GPU, gloo in the CPU tests); then every rank applies the same Adam update.
+
+The descriptor scaler (Eq. 2) is a min/max over every loaded atom: `allreduce_scaler` reduces the per-rank ranges.
+No arithmetic of the method lives here: the kernels are behind include/nep.h.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+
+def shard_structures(n_atoms: Sequence[int], world: int, work: Optional[Sequence[float]] = None) -> np.ndarray:
+    """owner[s] in 0..world-1 for every structure.  Longest-processing-time greedy on `work` (default: atoms per structure,
+    a proxy for its pair count), ties broken by structure id, so every rank computes the same table without communication."""
+    n_atoms = np.asarray(n_atoms, dtype=np.int64)
+    w = np.asarray(work if work is not None else n_atoms, dtype=np.float64)
+    if w.shape != n_atoms.shape:
+        raise ValueError("work must have one entry per structure")
+    if world < 1:
+        raise ValueError("world must be >= 1")
+    owner = np.zeros(len(n_atoms), dtype=np.int32)
+    load = np.zeros(world, dtype=np.float64)
+    order = np.lexsort((np.arange(len(w)), -w))          # heaviest first, then by id
+    for s in order:
+        r = int(np.argmin(load))                         # first minimum: deterministic
+        owner[s] = r
+        load[r] += w[s]
+    return owner
+
+
+@dataclass
+class Shard:
+    rank: int
+    world: int
+    owner: np.ndarray        # [S] owner of every structure
+    global_ids: np.ndarray   # [S_local] global ids of this rank's structures, ascending
+    local_of: np.ndarray     # [S] local id on its owner
+
+    @classmethod
+    def make(cls, n_atoms: Sequence[int], rank: int, world: int, work: Optional[Sequence[float]] = None) -> "Shard":
+        owner = shard_structures(n_atoms, world, work)
+        local_of = np.zeros(len(owner), dtype=np.int32)
+        for r in range(world):
+            ids = np.nonzero(owner == r)[0]
+            local_of[ids] = np.arange(len(ids), dtype=np.int32)
+        return cls(rank, world, owner, np.nonzero(owner == rank)[0].astype(np.int32), local_of)
+
+    def local_batch(self, batch_ids: Sequence[int]) -> np.ndarray:
+        """Local structure ids (order of the batch kept) of the part of a global batch that this rank owns."""
+        b = np.asarray(batch_ids, dtype=np.int64)
+        mine = b[self.owner[b] == self.rank]
+        return self.local_of[mine].astype(np.int32)
+
+
+def batch_normalisers(batch_ids: Sequence[int], n_atoms: Sequence[int], has_virial: Optional[Sequence[int]] = None):
+    """(S_b, N_b, S_v) of the whole batch: the counts Eqs. 5-7 divide by.  Every rank knows n_atoms and has_virial of the
+    whole data set (metadata), so no communication is needed."""
+    b = np.asarray(batch_ids, dtype=np.int64)
+    n = np.asarray(n_atoms, dtype=np.int64)
+    hv = np.ones(len(n), dtype=np.int64) if has_virial is None else np.asarray(has_virial, dtype=np.int64)
+    return int(len(b)), int(n[b].sum()), int(hv[b].sum())
+
+
+def allreduce_grad_loss(g, loss4, group=None):
+    """The step's one exchange: in-place sum over the ranks of the gradient and of the four loss terms."""
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)
+        dist.all_reduce(loss4, op=dist.ReduceOp.SUM, group=group)
+    return g, loss4
+
+
+def allreduce_scaler(qmin, qmax, group=None):
+    """Eq. 2 over every rank's atoms: s = 1 / (max - min) of the global ranges (degenerate range -> 1, DESIGN G10)."""
+    import torch
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(qmin, op=dist.ReduceOp.MIN, group=group)
+        dist.all_reduce(qmax, op=dist.ReduceOp.MAX, group=group)
+    rng = qmax - qmin
+    big = torch.maximum(qmax.abs(), qmin.abs()).clamp_min(1.0)
+    return torch.where(rng > 1e-12 * big, 1.0 / rng, torch.ones_like(rng))
+
+
+class DataParallelNep:
+    """A `Nep` context holding this rank's share of a structure set, driven with GLOBAL structure ids."""
+
+    def __init__(self, model, structures, rank: int, world: int, group=None, **kw):
+        from .binding import Nep
+        self.group = group
+        self.n_atoms = np.asarray(structures.n_atoms, dtype=np.int64)
+        self.shard = Shard.make(self.n_atoms, rank, world)
+        self.has_virial = np.ones(len(self.n_atoms), dtype=np.int64)
+        self.nep = Nep.from_model(model, **kw)
+        self.structures = structures
+        self._whole = (0, 0, 0)
+
+    def load(self, E=None, F=None, W=None, has_virial=None):
+        """Loads this rank's structures (labels optional, global arrays in the caller's order)."""
+        st = self.structures
+        sub = st.subset(self.shard.global_ids)
+        if has_virial is not None:
+            self.has_virial = np.asarray(has_virial, dtype=np.int64)
+        if E is None:
+            self.nep.load_structure_set(sub)
+        else:
+            off = np.concatenate([[0], np.cumsum(self.n_atoms)])
+            rows = np.concatenate([np.arange(off[s], off[s + 1]) for s in self.shard.global_ids]) if len(self.shard.global_ids) else np.zeros(0, np.int64)
+            hv = None if has_virial is None else np.asarray(has_virial, dtype=np.uint8)[self.shard.global_ids]
+            self.nep.load_structure_set(sub, np.asarray(E)[self.shard.global_ids], np.asarray(F)[rows], np.asarray(W)[self.shard.global_ids], hv)
+        self.nep.build_neighbors()
+
+    def set_batch(self, batch_ids: Sequence[int]):
+        self.nep.set_batch(self.shard.local_batch(batch_ids))
+        self._whole = batch_normalisers(batch_ids, self.n_atoms, self.has_virial)
+        self.nep.set_batch_normalisers(*self._whole)
+
+    def step(self, lam, lr: float, fetch_loss: bool = False):
+        """One training step on the current batch: forward, loss + gradient, the all-reduce, Adam."""
+        self.nep.forward_device()
+        self.nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
+        g, l4 = self.nep.grad_loss_tensors()
+        allreduce_grad_loss(g, l4, self.group)
+        self.nep.adam_step(lr)
+        return l4.cpu().numpy() if fetch_loss else None
