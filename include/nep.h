@@ -166,6 +166,9 @@ int nep_synchronize(nep_ctx* ctx);
  * of kernels through *n. */
 int nep_launch_count(nep_ctx* ctx, int64_t* n);
 int nep_profile_enable(nep_ctx* ctx, int on);
+/* While paused no events are recorded (no synchronisation, accumulators kept): lets a caller time kernels on a sample
+ * of its steps only, so that the event records do not sit between the kernels of every step. */
+int nep_profile_pause(nep_ctx* ctx, int paused);
 int nep_profile_read(nep_ctx* ctx, int cap, const char** names, double* ms, int64_t* launches, int* n);
 
 /* Sizes of the loaded set / current batch: {S, N, P_R, P_A, S_b, N_b, P_R_b, P_A_b}. */

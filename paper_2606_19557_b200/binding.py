@@ -56,6 +56,7 @@ SIGNATURES = {
     "nep_synchronize": (C.c_int, [_P]),
     "nep_launch_count": (C.c_int, [_P, C.POINTER(C.c_int64)]),
     "nep_profile_enable": (C.c_int, [_P, C.c_int]),
+    "nep_profile_pause": (C.c_int, [_P, C.c_int]),
     "nep_profile_read": (C.c_int, [_P, C.c_int, _P, _P, _P, C.POINTER(C.c_int)]),
     "nep_get_sizes": (C.c_int, [_P, _P]),
 }
@@ -333,6 +334,9 @@ class Nep:
 
     def profile_enable(self, on: bool = True):
         self._ck(self._L.nep_profile_enable(self._h, int(on)))
+
+    def profile_pause(self, paused: bool = True):
+        self._ck(self._L.nep_profile_pause(self._h, int(paused)))
 
     def profile_read(self, cap: int = 64):
         """{kernel name: (total ms, launches)} since the last read."""

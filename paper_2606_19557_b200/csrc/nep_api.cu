@@ -41,7 +41,7 @@ void dev_free(nep_ctx* c, void* p)
 void prof_begin(nep_ctx* c, const char* name)
 {
     ++c->launches;
-    if (!c->prof.on) return;
+    if (!c->prof.on || c->prof.paused) return;
     Profiler::Rec r; r.name = name;
     auto get = [&]() { cudaEvent_t e; if (!c->prof.pool.empty()) { e = c->prof.pool.back(); c->prof.pool.pop_back(); } else cudaEventCreate(&e); return e; };
     r.a = get(); r.b = get();
@@ -50,7 +50,7 @@ void prof_begin(nep_ctx* c, const char* name)
 }
 void prof_end(nep_ctx* c)
 {
-    if (!c->prof.on) return;
+    if (!c->prof.on || c->prof.paused) return;
     cudaEventRecord(c->prof.pending.back().b, c->stream);
 }
 
@@ -674,7 +674,13 @@ int nep_profile_enable(nep_ctx* c, int on)
     cudaStreamSynchronize(c->stream);
     for (auto& r : c->prof.pending) { c->prof.pool.push_back(r.a); c->prof.pool.push_back(r.b); }
     c->prof.pending.clear(); c->prof.acc.clear();
-    c->prof.on = on != 0;
+    c->prof.on = on != 0; c->prof.paused = false;
+    return NEP_OK;
+}
+int nep_profile_pause(nep_ctx* c, int paused)
+{
+    CHECK_CTX(c);
+    c->prof.paused = paused != 0;
     return NEP_OK;
 }
 int nep_profile_read(nep_ctx* c, int cap, const char** names, double* ms, int64_t* launches, int* n)

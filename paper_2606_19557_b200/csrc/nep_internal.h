@@ -102,6 +102,7 @@ struct BatchDev {
 
 struct Profiler {
     bool on = false;
+    bool paused = false;   // events are skipped while paused (the accumulators are kept)
     struct Rec { cudaEvent_t a, b; const char* name; };
     std::vector<Rec> pending;
     std::map<std::string, std::pair<double, int64_t>> acc;
