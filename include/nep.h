@@ -139,7 +139,7 @@ int nep_get_descriptors(nep_ctx* ctx, float* q);
 int nep_loss_grad(nep_ctx* ctx, double lambda_E, double lambda_F, double lambda_V, double* loss4_host);
 int nep_get_loss(nep_ctx* ctx, double* loss4_host);
 
-/* Data-parallel training over several contexts, one per GPU (DESIGN.md section 12).  Structures interact only with
+/* Data-parallel training over several contexts, one per GPU (DESIGN.md section 11).  Structures interact only with
  * themselves (Eq. 1), so the batch of a step is split by structure: every context holds its share of the data
  * set and calls nep_set_batch with its share of the batch.  The loss of Eq. 4 and its gradient (Eq. 8) are sums over
  * structures and atoms divided by the batch counts of Eqs. 5-7, so with the counts of the WHOLE batch given here

@@ -1,4 +1,4 @@
-"""Data-parallel NEP training over several GPUs, one process (rank) per GPU (DESIGN.md section 12; SURVEY section 8(e)).
+"""Data-parallel NEP training over several GPUs, one process (rank) per GPU (DESIGN.md section 11; SURVEY section 8(e)).
 
 Structures interact only with themselves (Eq. 1; the sums of Eqs. 15-20 run over the neighbours inside one
 periodic structure), so the units that shard are STRUCTURES:

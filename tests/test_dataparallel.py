@@ -1,4 +1,4 @@
-"""Data-parallel path (DESIGN.md section 12): structure sharding, whole-batch normalisers, the one all-reduce.
+"""Data-parallel path (DESIGN.md section 11): structure sharding, whole-batch normalisers, the one all-reduce.
 
 CPU tests (gloo, world_size 2): the host logic of paper_2606_19557_b200/dataparallel.py and the claim the C call
 nep_set_batch_normalisers rests on -- with the counts of Eqs. 5-7 taken over the whole batch, the loss terms and the
