@@ -12,7 +12,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
     const ModelDev& m = a.m;
     constexpr int CST = CoefStride<NCH, K>::value;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
-    float* cs = smem + SWEEP_SMEM_BYTES / 4;
+    float* cs = smem + SWEEP2_SMEM_BYTES / 4;
     const int n0 = blockIdx.y * NCH;
     load_cA_chunk<NCH, K>(a, cs, n0);
     __syncthreads();
@@ -33,10 +33,18 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
     const float rcinv = m.rcinvA;
     float* Fb = a.b.F;
     const int bbase = L.bbase;
-    sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
-        const PairGeo p = pair_geo(rc4);
-        float g[NCH], dg[NCH];
-        radial_gn<NCH, K, true>(p.r, rcinv, cbase + p.tj * CST, g, dg);
+    // two pairs per iteration (sweep_pairs2): the scalar chains of both are issued together, then the two contractions
+    struct Prep { PairGeo p; float g[NCH], dg[NCH]; };
+    auto prep = [&](const float4& rc4, float on) {
+        Prep P;
+        P.p = pair_geo(rc4);
+        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, P.dg);
+#pragma unroll
+        for (int n = 0; n < NCH; ++n) { P.g[n] *= on; P.dg[n] *= on; }
+        return P;
+    };
+    auto contract = [&](const Prep& P) {
+        const PairGeo& p = P.p;
         float b[NL], A[NL];
         float2 b2[NL / 2], A2[NL / 2];
         const HarmZ hz = harm_z(p.z);
@@ -49,13 +57,13 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
 #pragma unroll
         for (int n = 0; n < NCH; ++n) {
             float2 eb = make_float2(0.0f, 0.0f);
-            const float2 gg = dup2(g[n]);
+            const float2 gg = dup2(P.g[n]);
 #pragma unroll
             for (int l = 0; l < NL / 2; ++l) {
                 eb = __ffma2_rn(E2[n][l], b2[l], eb);
                 A2[l] = __ffma2_rn(gg, E2[n][l], A2[l]);
             }
-            radial = fmaf(dg[n], eb.x + eb.y, radial);
+            radial = fmaf(P.dg[n], eb.x + eb.y, radial);
         }
         unpack24(A2, A);
         float vx, vy, vz;
@@ -71,6 +79,11 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
         w[0] = fmaf(-p.dx, px, w[0]); w[1] = fmaf(-p.dx, py, w[1]); w[2] = fmaf(-p.dx, pz, w[2]);
         w[3] = fmaf(-p.dy, px, w[3]); w[4] = fmaf(-p.dy, py, w[4]); w[5] = fmaf(-p.dy, pz, w[5]);
         w[6] = fmaf(-p.dz, px, w[6]); w[7] = fmaf(-p.dz, py, w[7]); w[8] = fmaf(-p.dz, pz, w[8]);
+    };
+    sweep_pairs2<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+        const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
+        contract(A);
+        if (has2) contract(B);
     });
     if (L.ti >= 0) {
         float* Fi = sb_ptr(Fb, L.w, 3, L.lane);
@@ -89,7 +102,7 @@ int launch_ang_force(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
-        const size_t smem = SWEEP_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
+        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
         auto kern = k_ang_force<NCH, K>;
         if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         NEP_LAUNCH(c, "k_ang_force", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);

@@ -14,7 +14,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
     const ModelDev& m = a.m;
     constexpr int CST = CoefStride<NCH, K>::value;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
-    float* cs = smem + SWEEP_SMEM_BYTES / 4;
+    float* cs = smem + SWEEP2_SMEM_BYTES / 4;
     float* cR = cs + m.T * m.T * CST;                 // [ti][tj][n][k] as in theta (chunk 0 only)
     const int n0 = blockIdx.y * NCH;
     load_cA_chunk<NCH, K>(a, cs, n0);
@@ -50,20 +50,30 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
         for (int l = 0; l < NL / 2; ++l) S2[n][l] = make_float2(0.0f, 0.0f);
     const float* cbase = cs + (L.ti > 0 ? L.ti : 0) * m.T * CST;
     const float rcinv = m.rcinvA;
-    sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
-        const PairGeo p = pair_geo(rc4);
-        float g[NCH];
-        radial_gn<NCH, K, false>(p.r, rcinv, cbase + p.tj * CST, g, nullptr);
+    // two pairs per iteration (sweep_pairs2): the scalar chains of both are issued together, then the two rank-1 updates
+    struct Prep { PairGeo p; float g[NCH]; };
+    auto prep = [&](const float4& rc4, float on) {
+        Prep P;
+        P.p = pair_geo(rc4);
+        radial_gn<NCH, K, false>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, nullptr);
+#pragma unroll
+        for (int n = 0; n < NCH; ++n) P.g[n] *= on;
+        return P;
+    };
+    auto accumulate = [&](const Prep& P) {
         float b[NL];
-        const HarmZ hz = harm_z(p.z);
-        const HarmXY hxy = harm_xy(p.x, p.y);
-        harm24(hz, hxy, b);
+        harm24(harm_z(P.p.z), harm_xy(P.p.x, P.p.y), b);
 #pragma unroll
         for (int n = 0; n < NCH; ++n) {
-            const float2 gg = make_float2(g[n], g[n]);
+            const float2 gg = make_float2(P.g[n], P.g[n]);
 #pragma unroll
             for (int l = 0; l < NL / 2; ++l) S2[n][l] = __ffma2_rn(gg, make_float2(b[2 * l], b[2 * l + 1]), S2[n][l]);
         }
+    };
+    sweep_pairs2<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+        const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
+        accumulate(A);
+        accumulate(B);
     });
     float S[NCH][NL];
 #pragma unroll
@@ -90,7 +100,7 @@ int launch_ang_fwd(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
-        const size_t smem = SWEEP_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.nR * m.KR);
+        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.nR * m.KR);
         auto kern = k_ang_fwd<NCH, K>;
         if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         NEP_LAUNCH(c, "k_ang_fwd", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);

@@ -12,7 +12,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
     const ModelDev& m = a.m;
     constexpr int CST = CoefStride<NCH, K>::value;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
-    float* cs = smem + SWEEP_SMEM_BYTES / 4;
+    float* cs = smem + SWEEP2_SMEM_BYTES / 4;
     const int n0 = blockIdx.y * NCH;
     load_cA_chunk<NCH, K>(a, cs, n0);
     __syncthreads();
@@ -33,24 +33,38 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
     const float rcinv = m.rcinvA;
     const float* ub = a.b.u;
     const int bbase = L.bbase;
-    sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
-        const PairGeo p = pair_geo(rc4);
-        const Tangent T = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
-        float g[NCH], dg[NCH];
-        radial_gn<NCH, K, true>(p.r, rcinv, cbase + p.tj * CST, g, dg);
+    // per pair: the scalar part (geometry, tangent, radial functions) ...
+    struct Prep { PairGeo p; Tangent T; float g[NCH], c[NCH]; };
+    auto prep = [&](const float4& rc4, float on) {
+        Prep P;
+        P.p = pair_geo(rc4);
+        P.T = pair_tangent(ub, bbase, P.p, uix, uiy, uiz, G);
+        float dg[NCH];
+        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, dg);
+#pragma unroll
+        for (int n = 0; n < NCH; ++n) { P.g[n] *= on; P.c[n] = dg[n] * P.T.t * on; }
+        return P;
+    };
+    // ... and the rank-1 update of the 5 x 24 tangent moments
+    auto accumulate = [&](const Prep& P) {
         float b[NL], bd[NL];
-        const HarmZ hz = harm_z(p.z);
-        const HarmXY hxy = harm_xy(p.x, p.y);
+        const HarmZ hz = harm_z(P.p.z);
+        const HarmXY hxy = harm_xy(P.p.x, P.p.y);
         harm24(hz, hxy, b);
-        harm24_tangent(hz, hxy, T.rx, T.ry, T.rz, bd);
+        harm24_tangent(hz, hxy, P.T.rx, P.T.ry, P.T.rz, bd);
         float2 b2[NL / 2], bd2[NL / 2];
         pack24(b, b2); pack24(bd, bd2);
 #pragma unroll
         for (int n = 0; n < NCH; ++n) {
-            const float2 cc = dup2(dg[n] * T.t), gg = dup2(g[n]);
+            const float2 cc = dup2(P.c[n]), gg = dup2(P.g[n]);
 #pragma unroll
             for (int l = 0; l < NL / 2; ++l) Sd2[n][l] = __ffma2_rn(cc, b2[l], __ffma2_rn(gg, bd2[l], Sd2[n][l]));
         }
+    };
+    sweep_pairs2<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+        const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
+        accumulate(A);
+        accumulate(B);
     });
     float Sd[NCH][NL];
 #pragma unroll
@@ -80,7 +94,7 @@ int launch_ang_tangent(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
-        const size_t smem = SWEEP_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
+        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
         auto kern = k_ang_tangent<NCH, K>;
         if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         NEP_LAUNCH(c, "k_ang_tangent", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);

@@ -119,6 +119,41 @@ __device__ __forceinline__ void sweep_pairs(const float4* __restrict__ rec, int 
     sweep_pairs(rec, width, cnt, stage, [](bool, const float4&) {}, body);
 }
 
+// Two slots per iteration: body2(record of slot s, record of slot s + 1, has_second) for s = 0, 2, 4, ... < cnt.
+// The dependent chains of a pair (distance, cutoff polynomial, Chebyshev recurrence) are long and a sweep runs two
+// warps per scheduler, so the arithmetic of two pairs is interleaved to fill the pipe.  When the lane has no second
+// record the first one is passed again with has_second = false (finite values that the body multiplies by zero).
+// stage: 4 staging cells per thread, SWEEP2_TB apart.
+constexpr int SWEEP2_TB = 64;
+constexpr int SWEEP2_SMEM_BYTES = SWEEP2_TB * 16 * 4;
+template <int TB, class Body2>
+__device__ __forceinline__ void sweep_pairs2(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body2&& body2)
+{
+#pragma unroll
+    for (int g = 0; g < 2; ++g) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+            if (2 * g + h < width) cp_async16(stage + (2 * g + h) * TB, rec + (size_t)(2 * g + h) * WARP);
+        cp_async_commit();
+    }
+    for (int s = 0; s < width; s += 2) {
+        cp_async_wait<1>();
+        float4* c0 = stage + (s & 3) * TB;
+        float4* c1 = stage + ((s + 1) & 3) * TB;
+        const float4 r0 = *c0;
+        float4 r1 = *c1;
+        if (s + 4 < width) cp_async16(c0, rec + (size_t)(s + 4) * WARP);
+        if (s + 5 < width) cp_async16(c1, rec + (size_t)(s + 5) * WARP);
+        cp_async_commit();
+        if (s < cnt) {
+            const bool has2 = s + 1 < cnt;
+            if (!has2) r1 = r0;
+            body2(r0, r1, has2);
+        }
+    }
+    cp_async_wait<0>();
+}
+
 struct SweepA { const float4* rec; int width, cnt; };
 __device__ __forceinline__ SweepA sweep_init(const int64_t* __restrict__ recoff, const float4* __restrict__ recs,
                                              const int* __restrict__ cntp, const Lane& L)

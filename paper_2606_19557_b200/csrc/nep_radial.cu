@@ -33,7 +33,7 @@ __device__ __forceinline__ void sweep_pairs_rad(const float4* __restrict__ rec, 
 template <int K>
 __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
 {
-    __shared__ __align__(16) float4 stage_s[RAD_TB * SWEEP_STAGES];
+    __shared__ __align__(16) float4 stage_s[RAD_TB * 4];
     Lane L;
     if (!lane_init(a, L)) return;
     const ModelDev& m = a.m;
@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
     const float* arow_i = arow + (size_t)L.ib * TKRP;
     const int ti = L.ti, bbase = L.bbase;
     const float rcinv = m.rcinvR;
-    sweep_pairs_rad(sw.rec, sw.width, sw.cnt, stage_s + threadIdx.x, [](bool, const float4&) {}, [&](const float4& rc4) {
+    auto one = [&](const float4& rc4) {
         const PairGeo p = pair_geo(rc4);
         if (p.tj != cur) {
             cur = p.tj;
@@ -76,6 +76,10 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
         const float px = sij * p.x, py = sij * p.y, pz = sij * p.z;
         wxx = fmaf(-p.dx, px, wxx); wyy = fmaf(-p.dy, py, wyy); wzz = fmaf(-p.dz, pz, wzz);
         wxy = fmaf(-p.dx, py, wxy); wxz = fmaf(-p.dx, pz, wxz); wyz = fmaf(-p.dy, pz, wyz);
+    };
+    sweep_pairs2<RAD_TB>(sw.rec, sw.width, sw.cnt, stage_s + threadIdx.x, [&](const float4& ra, const float4& rb, bool has2) {
+        one(ra);
+        if (has2) one(rb);
     });
     float* Fi = sb_ptr(a.b.F, L.w, 3, L.lane);
     Fi[0] = fx; Fi[WARP] = fy; Fi[2 * WARP] = fz;
@@ -93,7 +97,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
 template <int K>
 __global__ void __launch_bounds__(RAD_TB) k_rad_tangent(StepArgs a)
 {
-    __shared__ __align__(16) float4 stage_s[RAD_TB * SWEEP_STAGES];
+    __shared__ __align__(16) float4 stage_s[RAD_TB * 4];
     Lane L;
     if (!lane_init(a, L)) return;
     const ModelDev& m = a.m;
@@ -119,7 +123,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_tangent(StepArgs a)
     const float* ub = a.b.u;
     const int bbase = L.bbase;
     const float rcinv = m.rcinvR;
-    sweep_pairs_rad(sw.rec, sw.width, sw.cnt, stage_s + threadIdx.x, [](bool, const float4&) {}, [&](const float4& rc4) {
+    auto one = [&](const float4& rc4) {
         const PairGeo p = pair_geo(rc4);
         if (p.tj != cur) {
             if (cur >= 0) store();
@@ -127,6 +131,10 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_tangent(StepArgs a)
         }
         const Tangent T = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
         cheb_basis<K, true>(p.r, rcinv, [&](int k, float, float dfk) { bd[k] = fmaf(dfk, T.t, bd[k]); });
+    };
+    sweep_pairs2<RAD_TB>(sw.rec, sw.width, sw.cnt, stage_s + threadIdx.x, [&](const float4& ra, const float4& rb, bool has2) {
+        one(ra);
+        if (has2) one(rb);
     });
     if (cur >= 0) store();
 }
