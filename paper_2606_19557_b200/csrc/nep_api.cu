@@ -499,7 +499,8 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
         if (ids) { if (seen[s]) return fail(c, NEP_EINVAL, "duplicate structure id in batch"); seen[s] = 1; }
         nbs64 += (c->h_pbase[s + 1] - c->h_pbase[s]) / WARP;
     }
-    if (nbs64 * WARP > INT32_MAX / 2) return fail(c, NEP_ECAPACITY, "batch too large");
+    if (nbs64 * WARP > INT32_MAX / 2 || nbs64 * WARP * c->m.T * c->m.KRP > (int64_t)UINT32_MAX)
+        return fail(c, NEP_ECAPACITY, "batch too large");   // 32-bit element indices into the per-atom rows
     const int nbs = (int)nbs64;
     // network tiles: atoms sorted by species, every species padded to whole tiles
     const int TM = ann_tile_m(c);
