@@ -1,0 +1,147 @@
+"""Epoch driver around the training step (paper P:99-103, Fig. 1, Table I).
+
+Host logic only -- every number is produced by the kernels behind include/nep.h:
+
+  * mini-batches : a seeded permutation of the structure ids per epoch, cut into batches of `batch` structures;
+  * two stages   : (lambda_E, lambda_F, lambda_V, lr) switch at epoch `start_stage2` (Table I "Stage II"); the plateau
+                   counter and the best loss restart with the stage, the learning rate restarts at `stage2_lr`;
+  * plateau decay: ReduceLROnPlateau on the epoch-mean training loss, Eq. 14: eta_{e+1} = max(gamma eta_e, eta_min)
+                   whenever the loss has not improved for `patience` consecutive epochs; the rate is constant inside an
+                   epoch.  "Improved" = below best * (1 - threshold) (the relative mode of the scheduler the paper names,
+                   reading: the paper gives gamma and p only; threshold 1e-4 is that scheduler's default);
+  * reporting    : epoch-mean loss terms and, on request, RMSEs of energy per atom, force components and virial per atom.
+"""
+from __future__ import annotations
+
+import dataclasses
+from typing import Callable, List, Optional, Sequence, Tuple
+
+import numpy as np
+
+
+@dataclasses.dataclass
+class StageSpec:
+    lr: float
+    lambda_e: float
+    lambda_f: float
+    lambda_v: float
+
+
+@dataclasses.dataclass
+class TrainConfig:
+    """Names follow Table I of the paper."""
+    epoch: int = 600
+    batch: int = 16
+    stage1: StageSpec = dataclasses.field(default_factory=lambda: StageSpec(5e-3, 1.0, 100.0, 1.0))
+    stage2: Optional[StageSpec] = dataclasses.field(default_factory=lambda: StageSpec(5e-4, 100.0, 5.0, 30.0))
+    start_stage2: int = 300
+    scheduler_patience: int = 15
+    scheduler_factor: float = 0.5
+    scheduler_threshold: float = 1e-4
+    min_lr: float = 1e-6
+    seed: int = 0
+    adam_variant: int = 0          # 0: Eqs. 9-13 literally; 1: torch.optim.Adam(amsgrad=True)
+
+    def stage_of(self, epoch: int) -> Tuple[int, StageSpec]:
+        if self.stage2 is not None and epoch >= self.start_stage2:
+            return 2, self.stage2
+        return 1, self.stage1
+
+
+class PlateauSchedule:
+    """Eq. 14: the learning rate of the next epoch from the epoch-mean losses seen so far."""
+
+    def __init__(self, lr: float, factor: float, patience: int, min_lr: float, threshold: float = 1e-4):
+        if not (0.0 < factor < 1.0):
+            raise ValueError("gamma must lie in (0, 1)")
+        self.lr, self.factor, self.patience, self.min_lr, self.threshold = float(lr), factor, int(patience), float(min_lr), threshold
+        self.best = float("inf")
+        self.bad = 0
+
+    def step(self, loss: float) -> float:
+        if loss < self.best * (1.0 - self.threshold):
+            self.best = loss
+            self.bad = 0
+        else:
+            self.bad += 1
+        if self.bad > self.patience:
+            self.lr = max(self.factor * self.lr, self.min_lr)
+            self.bad = 0
+        return self.lr
+
+
+def epoch_batches(n_struct: int, batch: int, seed: int, epoch: int) -> List[np.ndarray]:
+    """Seeded permutation of the structure ids of one epoch, cut into consecutive batches (the last may be smaller)."""
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([int(seed), int(epoch)])))
+    perm = rng.permutation(n_struct).astype(np.int32)
+    return [perm[i:i + batch] for i in range(0, n_struct, batch)]
+
+
+@dataclasses.dataclass
+class EpochRecord:
+    epoch: int
+    stage: int
+    lr: float
+    loss: float
+    dE: float
+    dF: float
+    dV: float
+
+
+class Trainer:
+    """Drives a loaded `Nep` context (structures, labels, neighbour lists, parameters and scaler already set)."""
+
+    def __init__(self, nep, cfg: TrainConfig):
+        self.nep, self.cfg = nep, cfg
+        self.history: List[EpochRecord] = []
+        self._sched: Optional[PlateauSchedule] = None
+        self._stage = 0
+
+    def _enter(self, stage: int, spec: StageSpec):
+        self._stage = stage
+        self._sched = PlateauSchedule(spec.lr, self.cfg.scheduler_factor, self.cfg.scheduler_patience, self.cfg.min_lr,
+                                      self.cfg.scheduler_threshold)
+
+    def run_epoch(self, epoch: int) -> EpochRecord:
+        cfg, nep = self.cfg, self.nep
+        stage, spec = cfg.stage_of(epoch)
+        if stage != self._stage:
+            self._enter(stage, spec)
+        lr = self._sched.lr
+        sums = np.zeros(4)
+        nb = 0
+        for ids in epoch_batches(nep.n_struct, cfg.batch, cfg.seed, epoch):
+            nep.set_batch(ids)
+            nep.forward_device()
+            sums += nep.loss_grad(spec.lambda_e, spec.lambda_f, spec.lambda_v, fetch_loss=True)
+            nep.adam_step(lr, variant=cfg.adam_variant)
+            nb += 1
+        mean = sums / max(nb, 1)
+        self._sched.step(float(mean[0]))          # takes effect from the next epoch (Eq. 14)
+        rec = EpochRecord(epoch, stage, lr, float(mean[0]), float(mean[1]), float(mean[2]), float(mean[3]))
+        self.history.append(rec)
+        return rec
+
+    def fit(self, epochs: Optional[int] = None, callback: Optional[Callable[[EpochRecord], None]] = None) -> List[EpochRecord]:
+        for e in range(len(self.history), epochs if epochs is not None else self.cfg.epoch):
+            rec = self.run_epoch(e)
+            if callback:
+                callback(rec)
+        return self.history
+
+    def rmse(self, n_atoms: Sequence[int], E: np.ndarray, F: np.ndarray, W: np.ndarray, chunk: int = 1024) -> dict:
+        """Root-mean-square errors over the whole loaded set: energy and virial per atom, force per component."""
+        nep = self.nep
+        n_atoms = np.asarray(n_atoms, dtype=np.int64)
+        off = np.concatenate([[0], np.cumsum(n_atoms)])
+        se = sf = sv = 0.0
+        for i in range(0, nep.n_struct, chunk):
+            ids = np.arange(i, min(i + chunk, nep.n_struct), dtype=np.int32)
+            nep.set_batch(ids)
+            Eg, Fg, Wg = nep.forward()
+            n = n_atoms[ids].astype(np.float64)
+            se += float(np.sum(((Eg - E[ids]) / n) ** 2))
+            sv += float(np.sum(((Wg - W[ids]) / n[:, None]) ** 2))
+            sf += float(np.sum((Fg - F[off[ids[0]]:off[ids[-1] + 1]]) ** 2))
+        S, N = nep.n_struct, int(n_atoms.sum())
+        return {"energy_per_atom": (se / S) ** 0.5, "force": (sf / (3 * N)) ** 0.5, "virial_per_atom": (sv / (9 * S)) ** 0.5}
