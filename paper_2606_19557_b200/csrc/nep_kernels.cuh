@@ -70,7 +70,7 @@ __device__ __forceinline__ PairGeo pair_geo(const float4& rec)
     const int bits = __float_as_int(rec.w);
     p.jl = bits & 0xffffff; p.tj = bits >> 24;
     const float r2 = fmaf(p.dx, p.dx, fmaf(p.dy, p.dy, p.dz * p.dz));
-    p.rinv = rsqrtf(r2);
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(p.rinv) : "f"(r2));   // r2 is never subnormal: skip rsqrtf's scaling path
     p.r = r2 * p.rinv;
     p.x = p.dx * p.rinv; p.y = p.dy * p.rinv; p.z = p.dz * p.rinv;
     return p;
