@@ -346,12 +346,12 @@ def run_ours(args):
             roof = {"kernel": top, "bound": "hbm", "achieved": mdl["bytes"] / dur / 1e9, "peak": hbm_peak, "unit": "GB/s", "peak_source": peak_src}
         roof["frac"] = roof["achieved"] / roof["peak"]
         roof["traffic"] = None
-        tpath = os.path.join(ROOT, "profiles", "r01c_traffic.json")   # DRAM bytes per launch from the committed ncu capture
+        tpath = os.path.join(ROOT, "profiles", "r01d_traffic.json")   # DRAM bytes per launch from the committed ncu capture
         if os.path.exists(tpath):
             tj = json.load(open(tpath))
             if tj.get("workload") == f"config{w.config_id}" and args.n_struct is None:
                 roof["traffic"] = tj["bytes_per_launch"].get(top)
-                roof["traffic_source"] = "profiles/r01c_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
+                roof["traffic_source"] = "profiles/r01d_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
         roof["share_of_step"] = kern[top]["share"]
         roof["avg_ms"] = kern[top]["ms"]
         roof["algorithmic_flops_per_launch"] = mdl["flops"]
