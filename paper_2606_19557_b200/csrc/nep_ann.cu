@@ -455,36 +455,25 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
             atomicAdd(gt + which * m.H + mu, which ? s : -s);
         }
     }
-    {   // g_w0[t][mu][v] += s_v sum_atoms (gamma_mu q_v + e_mu qd_v) : thread = rows {ra + RS jr} x cols {cb + 8 jc}
-        constexpr int RS = NT / 8;
+    if (tid < 128) {
+        // g_w0[t][mu][v] += s_v sum_atoms (gamma_mu q_v + e_mu qd_v): 2 rows {ra, ra + 16} x 5 columns {cb + 8 c} per thread on
+        // four warps: 14 shared-memory loads per 80 FFMA (one row per thread on all eight warps: 12 per 40)
         const int ra = tid >> 3, cb = tid & 7;
         float* gt = a.g + (size_t)t * m.per_type;
-        const int nrg = (l.HP8 + RS - 1) / RS;          // row groups that hold real rows (rows up to HP32 are zero)
-        for (int jr0 = 0; jr0 < nrg; jr0 += 2) {
-            const bool two = jr0 + 1 < nrg;
-            const int r0 = ra + RS * jr0;
+        for (int rb = 0; rb < l.HP8; rb += 32) {
+            const int r0 = rb + ra;
             for_chunks(l.DP8 / 8, [&](int jc0, auto cwc) {
                 constexpr int CW = decltype(cwc)::value;
                 const int c0 = cb + 8 * jc0;
-                if (two) {
-                    float acc[2][CW];
-                    outer_gemm<2, CW>(sm + l.Gs + r0 * LD, sm + l.Es + r0 * LD, RS * LD, sm + l.Qs + c0 * LD, sm + l.QDs + c0 * LD, 8 * LD, TM, acc);
+                float acc[2][CW];
+                outer_gemm<2, CW>(sm + l.Gs + r0 * LD, sm + l.Es + r0 * LD, 16 * LD, sm + l.Qs + c0 * LD, sm + l.QDs + c0 * LD, 8 * LD, TM, acc);
 #pragma unroll
-                    for (int r = 0; r < 2; ++r)
-#pragma unroll
-                        for (int cc = 0; cc < CW; ++cc) {
-                            const int mu = r0 + RS * r, v = c0 + 8 * cc;
-                            if (mu < m.H && v < m.D) atomicAdd(gt + mu * m.D + v, sm[l.sc + v] * acc[r][cc]);
-                        }
-                } else {
-                    float acc[1][CW];
-                    outer_gemm<1, CW>(sm + l.Gs + r0 * LD, sm + l.Es + r0 * LD, RS * LD, sm + l.Qs + c0 * LD, sm + l.QDs + c0 * LD, 8 * LD, TM, acc);
+                for (int r = 0; r < 2; ++r)
 #pragma unroll
                     for (int cc = 0; cc < CW; ++cc) {
-                        const int v = c0 + 8 * cc;
-                        if (r0 < m.H && v < m.D) atomicAdd(gt + r0 * m.D + v, sm[l.sc + v] * acc[0][cc]);
+                        const int mu = r0 + 16 * r, v = c0 + 8 * cc;
+                        if (mu < m.H && v < m.D) atomicAdd(gt + mu * m.D + v, sm[l.sc + v] * acc[r][cc]);
                     }
-                }
             });
         }
     }
