@@ -175,14 +175,12 @@ def e2e_step(nep, lam, ids):
     nep.set_batch(ids)
     dp_whole_batch(nep)
     nep.forward_device()
+    nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
+    dp_exchange(nep)
+    nep.adam_step(LR)                              # queued before the read-back below synchronises
     if DP["views"] is None:
-        l4 = nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=True)
-    else:
-        nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
-        dp_exchange(nep)
-        l4 = DP["views"][1].cpu().numpy()          # the whole batch's loss terms -> host
-    nep.adam_step(LR)
-    return l4
+        return nep.get_loss()                      # the step's loss terms -> host
+    return DP["views"][1].cpu().numpy()            # the whole batch's loss terms -> host
 
 
 def run_ours(args):
@@ -369,7 +367,7 @@ def run_ours(args):
                    "device_bytes": nep.bytes_allocated, "parallelism": (f"dp{world}: structures sharded, whole batch = {world} x {w.batch_size} structures, one NCCL all-reduce of g "
                                     f"[{w.model.n_par} fp32] + 4 loss terms per step" if use_dist else "dp1 (one GPU, no collective)")},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
-                "what": "per step: nep_set_batch(host ids) + nep_forward + nep_loss_grad(loss -> host) + nep_adam_step; geometry cache resident (P:143)"},
+                "what": "per step: nep_set_batch(host ids) + nep_forward + nep_loss_grad + nep_adam_step + nep_get_loss(-> host); geometry cache resident (P:143)"},
         "gpu_launches": int(launches),
         "clocks": clk,
         "roofline": roof,

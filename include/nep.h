@@ -137,7 +137,7 @@ int nep_get_descriptors(nep_ctx* ctx, float* q);
  * and parameters immediately before (NEP_ESTATE otherwise) and labels.  loss4_host: {L, dE, dF, dV} as
  * doubles on the host (synchronises) or NULL (stays on the device; see nep_get_loss). */
 int nep_loss_grad(nep_ctx* ctx, double lambda_E, double lambda_F, double lambda_V, double* loss4_host);
-int nep_get_loss(nep_ctx* ctx, double* loss4_host);
+int nep_get_loss(nep_ctx* ctx, double* loss4_host);   /* valid until the next nep_forward, also after nep_adam_step */
 
 /* Data-parallel training over several contexts, one per GPU.  Structures interact only with
  * themselves (Eq. 1), so the batch of a step is split by structure: every context holds its share of the data

@@ -195,7 +195,7 @@ static void free_dataset(nep_ctx* c)
                            d.offR, d.jR, d.shR, d.offA, d.jA, d.shA, d.cntR, d.recoffR, d.recR, d.cntA, d.recoffA, d.recA, d.B };
     for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
     memset(&d, 0, sizeof d);
-    c->have_data = c->have_labels = c->have_nbrs = c->forward_valid = c->grad_valid = false;
+    c->have_data = c->have_labels = c->have_nbrs = c->forward_valid = c->grad_valid = c->loss_valid = false;
 }
 
 static int upload_labels(nep_ctx* c, const double* E, const double* F, const double* W, const unsigned char* hv)
@@ -566,7 +566,7 @@ int nep_forward(nep_ctx* c, void* E_out, void* F_out, void* W_out, int on_host)
     if (!c->have_scaler) return fail(c, NEP_ESTATE, "nep_forward before nep_set_scaler / nep_compute_scaler");
     int rc = launch_forward(c, false);
     if (rc) return rc;
-    c->forward_valid = true; c->grad_valid = false;
+    c->forward_valid = true; c->grad_valid = false; c->loss_valid = false;
     if (E_out || F_out || W_out) {
         const BatchDev& b = c->b;
         size_t nE = (size_t)b.Sb, nF = 3 * (size_t)b.Nb, nW = 9 * (size_t)b.Sb;
@@ -626,7 +626,7 @@ int nep_get_loss(nep_ctx* c, double* loss4)
 {
     CHECK_CTX(c);
     if (!loss4) return fail(c, NEP_EINVAL, "loss4 is NULL");
-    if (!c->grad_valid) return fail(c, NEP_ESTATE, "nep_get_loss needs nep_loss_grad first");
+    if (!c->loss_valid) return fail(c, NEP_ESTATE, "nep_get_loss needs nep_loss_grad first");
     return d2h(c, loss4, c->b.lacc + 4, 32);
 }
 
@@ -639,7 +639,7 @@ int nep_loss_grad(nep_ctx* c, double lambda_E, double lambda_F, double lambda_V,
     c->lamE = lambda_E; c->lamF = lambda_F; c->lamV = lambda_V;
     int rc = launch_loss_grad(c);
     if (rc) return rc;
-    c->grad_valid = true;
+    c->grad_valid = true; c->loss_valid = true;
     if (loss4_host) return d2h(c, loss4_host, c->b.lacc + 4, 32);
     return NEP_OK;
 }

@@ -131,7 +131,7 @@ struct nep_ctx {
     std::vector<int> h_type, h_slot_of;   // [N] species ; structure-local slot of every atom
     std::vector<float> h_Flab;            // [N][3] force labels in the caller's order (re-laid out when the slot order changes)
     bool have_data = false, have_labels = false, have_nbrs = false, have_params = false, have_scaler = false;
-    bool forward_valid = false, grad_valid = false;
+    bool forward_valid = false, grad_valid = false, loss_valid = false;   // loss_valid: the loss terms of the last nep_loss_grad are still on the device
     int64_t PR = 0, PA = 0;
 
     nep::DataDev d{};
