@@ -238,8 +238,9 @@ int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
             NEP_LAUNCH(c, "k_ang_adjoint", (k_ang_adjoint<NCH, K, false>), dim3((unsigned)((c->b.nbs + nw - 1) / nw), a.nchunks), nw * WARP, smem, a);
         } else {
             auto bytes = [&](int nw) { return (size_t)SWEEP_SMEM_BYTES + 4 * (size_t)nw * ((size_t)m.T * NK * ADJ_TST + m.T); };
-            // two warps per block while three such blocks fit in one SM's shared memory, else one
-            const int nw = (bytes(2) + 1024) * 3 <= 228 * 1024 ? 2 : 1;
+            // one warp per block: the per-lane table columns of a warp take up to 30 KB, and one-warp blocks fill the SM's
+            // shared memory in the finest steps (config 4: 7 instead of 6 warps per SM, 626 -> 597 us)
+            const int nw = 1;
             const size_t smem = bytes(nw);
             if (smem > (size_t)c->max_smem_optin) return fail(c, NEP_ECAPACITY, "angular coefficient tables do not fit in shared memory");
             auto kern = k_ang_adjoint<NCH, K, true>;
