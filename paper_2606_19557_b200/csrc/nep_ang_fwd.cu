@@ -15,11 +15,16 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
     constexpr int CST = CoefStride<NCH, K>::value;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
     float* cs = smem + SWEEP2_SMEM_BYTES / 4;
-    float* cR = cs + m.T * m.T * CST;                 // [ti][tj][n][k] as in theta (chunk 0 only)
+    float* cR = cs + m.T * m.T * CST;                 // chunk 0 only: radial coefficients transposed to [ti][tj][k][n], n padded to 4
+    const int nRP = (m.nR + 3) & ~3;
     const int n0 = blockIdx.y * NCH;
     load_cA_chunk<NCH, K>(a, cs, n0);
     if (blockIdx.y == 0)
-        for (int i = threadIdx.x; i < m.T * m.T * m.nR * m.KR; i += blockDim.x) cR[i] = a.theta[m.o_cR + i];
+#pragma unroll 8
+        for (int i = threadIdx.x; i < m.T * m.T * m.KR * nRP; i += blockDim.x) {
+            const int pt = i / (m.KR * nRP), rem = i - pt * m.KR * nRP, k = rem / nRP, n = rem - k * nRP;
+            cR[i] = n < m.nR ? __ldg(a.theta + m.o_cR + (pt * m.nR + n) * m.KR + k) : 0.0f;
+        }
     __syncthreads();
     Lane L;
     if (!lane_init(a, L)) return;
@@ -30,14 +35,34 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
         if (L.lane < 9) a.b.Ws[9 * L.sb + L.lane] = 0.0f;
         else if (L.lane == 9) a.b.Es[L.sb] = 0.0;
         const float* Bp = sb_ptr(a.d.B, L.ds, m.T * m.KR, L.lane);
-        for (int n = 0; n < m.nR; ++n) {
-            float acc = 0.0f;
+        // q_n = sum_{T', k} cR[t_i][T'][n][k] B_k[T']: every B value is loaded once and meets 8 channels in registers
+        for (int n0 = 0; n0 < m.nR; n0 += 8) {
+            float acc[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[j] = 0.0f;
             if (L.ti >= 0) {
-                const float* cc = cR + (L.ti * m.T * m.nR + n) * m.KR;
-                for (int tj = 0; tj < m.T; ++tj)
-                    for (int k = 0; k < m.KR; ++k) acc = fmaf(cc[tj * m.nR * m.KR + k], __ldg(Bp + (size_t)(tj * m.KR + k) * WARP), acc);
+                const bool two = n0 + 4 < nRP;
+                const float* cc = cR + (size_t)L.ti * m.T * m.KR * nRP + n0;   // rows r = T' * KR + k are nRP apart
+                const int TK = m.T * m.KR;
+                for (int r0 = 0; r0 < TK; r0 += 8) {
+                    float b[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) b[j] = r0 + j < TK ? __ldg(Bp + (size_t)(r0 + j) * WARP) : 0.0f;   // eight loads in flight
+#pragma unroll
+                    for (int j = 0; j < 8; ++j)
+                        if (r0 + j < TK) {
+                            const float4 c0 = *reinterpret_cast<const float4*>(cc + (r0 + j) * nRP);
+                            acc[0] = fmaf(c0.x, b[j], acc[0]); acc[1] = fmaf(c0.y, b[j], acc[1]); acc[2] = fmaf(c0.z, b[j], acc[2]); acc[3] = fmaf(c0.w, b[j], acc[3]);
+                            if (two) {
+                                const float4 c1 = *reinterpret_cast<const float4*>(cc + (r0 + j) * nRP + 4);
+                                acc[4] = fmaf(c1.x, b[j], acc[4]); acc[5] = fmaf(c1.y, b[j], acc[5]); acc[6] = fmaf(c1.z, b[j], acc[6]); acc[7] = fmaf(c1.w, b[j], acc[7]);
+                            }
+                        }
+                }
             }
-            qp[(size_t)n * WARP] = acc;
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (n0 + j < m.nR) qp[(size_t)(n0 + j) * WARP] = acc[j];
         }
     }
 
@@ -100,7 +125,7 @@ int launch_ang_fwd(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
-        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.nR * m.KR);
+        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.KR * ((m.nR + 3) & ~3));
         auto kern = k_ang_fwd<NCH, K>;
         if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         NEP_LAUNCH(c, "k_ang_fwd", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);

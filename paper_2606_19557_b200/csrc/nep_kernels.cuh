@@ -183,10 +183,12 @@ __device__ __forceinline__ void load_cA_chunk(const StepArgs& a, float* cs, int 
     const ModelDev& m = a.m;
     constexpr int NCHP = ChunkPad<NCH>::value, CST = CoefStride<NCH, K>::value;
     const int tot = m.T * m.T * CST;
+    // unrolled: the loads of eight elements are in flight together (at 5 species the table is ~1100 values per block)
+#pragma unroll 8
     for (int i = threadIdx.x; i < tot; i += blockDim.x) {
         const int pt = i / CST, rem = i - pt * CST, k = rem / NCHP, n = rem - k * NCHP;
         float v = 0.0f;
-        if (k < m.KA && n < NCH && n0 + n < m.nA) v = a.theta[m.o_cA + (pt * m.nA + n0 + n) * m.KA + k];
+        if (k < m.KA && n < NCH && n0 + n < m.nA) v = __ldg(a.theta + m.o_cA + (pt * m.nA + n0 + n) * m.KA + k);
         cs[i] = v;
     }
 }
