@@ -177,3 +177,46 @@ def test_harmonic_table_against_scipy_and_gradient_fd():
         fd = (O.angular_functions(u + e)[0] - O.angular_functions(u - e)[0]) / (2 * h)
         assert np.allclose(dbu[:, a], fd, atol=1e-8)
     assert np.allclose(dbu @ u, 0.0, atol=1e-12)             # tangential: functions of the direction only
+
+
+# ---- C6: the descriptor scaler of Eq. 2, reading G10 ----
+def test_scaler_closed_form_on_hand_built_columns():
+    """q_nu~ = q_nu / (q_nu^max - q_nu^min) (Eq. 2): the range is over every atom, all species together (Eq. 2 has
+    no species index), not the maximum alone; a constant column has no range and gets s = 1 (reading G10)."""
+    q = np.array([
+        # positive range | straddles zero | constant | two "species" mixed in one column | negative only
+        [2.0, -1.5, 0.75, 10.0, -4.0],
+        [5.0, 0.25, 0.75, 11.0, -1.0],
+        [3.5, 2.5, 0.75, -3.0, -2.5],
+        [4.0, 0.0, 0.75, -2.0, -3.0],
+    ])
+    s = O.scaler(q)
+    expect = np.array([1.0 / (5.0 - 2.0), 1.0 / (2.5 + 1.5), 1.0, 1.0 / (11.0 + 3.0), 1.0 / (-1.0 + 4.0)])
+    assert np.allclose(s, expect, rtol=1e-15, atol=0)
+    # the mutations a plausible slip would make all differ from the closed form on these columns
+    assert not np.allclose(expect, 1.0 / q.max(0))                                  # 1 / max
+    assert not np.allclose(expect, 1.0 / np.abs(q).max(0))                          # 1 / max |q|
+    per_species = 1.0 / np.minimum(np.ptp(q[:2], axis=0) + 1e-300, np.ptp(q[2:], axis=0) + 1e-300)
+    assert not np.allclose(expect[3], per_species[3])                               # per-species ranges (rows 0-1 / 2-3)
+    # scale covariance and shift invariance of a range
+    assert np.allclose(O.scaler(3.0 * q + 7.0)[[0, 1, 3, 4]], expect[[0, 1, 3, 4]] / 3.0, rtol=1e-14)
+    # one atom: every range is degenerate
+    assert np.array_equal(O.scaler(q[:1]), np.ones(5))
+
+
+def test_scaler_degenerate_threshold():
+    """Reading G10: range <= 1e-12 max(1, max|q|) counts as constant (s = 1); anything wider is inverted."""
+    q = np.array([[1.0, 1.0, 1e6, 1e6], [1.0 + 5e-13, 1.0 + 4e-12, 1e6 + 5e-7, 1e6 + 4e-6]])
+    s = O.scaler(q)
+    assert s[0] == 1.0 and s[2] == 1.0
+    assert np.isclose(s[1], 1.0 / (q[1, 1] - q[0, 1]), rtol=1e-12) and np.isclose(s[3], 1.0 / (q[1, 3] - q[0, 3]), rtol=1e-12)
+
+
+def test_scaler_of_descriptors_is_inverse_range(small):
+    """On a real descriptor matrix: s = 1 / ptp(q) over all atoms of all species (the set has 2 species)."""
+    model, st, th, q = small
+    assert len(np.unique(st.type)) == 2
+    s = O.scaler(q)
+    assert s.shape == (model.D,)
+    assert np.allclose(s, 1.0 / np.ptp(q, axis=0), rtol=1e-13)
+    assert np.allclose((q * s).max(0) - (q * s).min(0), 1.0, rtol=1e-12)            # q~ spans exactly one unit (Eq. 2)
