@@ -19,7 +19,8 @@
  *   - "host" pointers are plain host memory, borrowed for the duration of the call only.
  *     "device" pointers are CUDA device memory on the context's device.
  *   - Device memory is obtained through the caller's allocator callbacks (the Python binding
- *     implements them with torch tensors).  If `alloc` is NULL the library uses cudaMalloc/cudaFree.
+ *     implements them with torch tensors).  The library never calls cudaMalloc: alloc == NULL or
+ *     free_ == NULL is NEP_EINVAL.
  *   - Step calls (nep_forward / nep_loss_grad / nep_adam_step) enqueue work on the context's stream
  *     and return without synchronising unless a host output is requested.
  *   - There is no CPU fallback: without a CUDA device nep_create fails with NEP_ECUDA.
@@ -118,6 +119,15 @@ int nep_get_adam_state(nep_ctx* ctx, float* m, float* v, float* vmax, int64_t* t
 int nep_compute_scaler(nep_ctx* ctx);
 int nep_set_scaler(nep_ctx* ctx, const double* s);
 int nep_get_scaler(nep_ctx* ctx, double* s);
+/* Eq. 2 when the training set is spread over several contexts (data-parallel training, below): the range of Eq. 2 is
+ * over EVERY atom of the set, so each context reports the minimum and maximum of each descriptor component over its
+ * own atoms (qmin, qmax: D doubles each, host; +inf / -inf for a context without atoms), the caller reduces them
+ * over the contexts (element-wise min / max, e.g. two all-reduces) and hands the result to every context, which
+ * forms s = 1 / (max - min) itself (a component without a range gets s = 1, DESIGN G10).
+ * nep_compute_scaler == nep_compute_descriptor_range followed by nep_set_scaler_from_range on one context.
+ * Both select the full loaded set as the current batch. */
+int nep_compute_descriptor_range(nep_ctx* ctx, double* qmin, double* qmax);
+int nep_set_scaler_from_range(nep_ctx* ctx, const double* qmin, const double* qmax);
 
 /* Mini-batch = a list of structure ids ("batch" of Table I).  ids == NULL: the whole set.
  * ids are copied to the device; the same id must not appear twice. */
@@ -147,7 +157,7 @@ int nep_get_loss(nep_ctx* ctx, double* loss4_host);   /* valid until the next ne
  * every context produces its additive share of {L, dE, dF, dV} and of g.  The caller sums g [N_par floats] and the four
  * loss terms [4 doubles] over the contexts in place -- device pointers from nep_grad_device_ptr, e.g. one NCCL
  * all-reduce each -- and then calls nep_adam_step on every context (identical updates, no parameter broadcast).
- * nep_set_batch resets the counts to those of the local batch.  Call after nep_set_batch, before nep_loss_grad. */
+ * nep_set_batch and nep_set_labels reset the counts to those of the local batch.  Call after them, before nep_loss_grad. */
 int nep_set_batch_normalisers(nep_ctx* ctx, int64_t n_struct_whole, int64_t n_atoms_whole, int64_t n_virial_whole);
 int nep_grad_device_ptr(nep_ctx* ctx, float** g, double** loss4);
 

@@ -45,6 +45,8 @@ SIGNATURES = {
     "nep_compute_scaler": (C.c_int, [_P]),
     "nep_set_scaler": (C.c_int, [_P, _P]),
     "nep_get_scaler": (C.c_int, [_P, _P]),
+    "nep_compute_descriptor_range": (C.c_int, [_P, _P, _P]),
+    "nep_set_scaler_from_range": (C.c_int, [_P, _P, _P]),
     "nep_set_batch": (C.c_int, [_P, C.c_int, _P]),
     "nep_forward": (C.c_int, [_P, _P, _P, _P, C.c_int]),
     "nep_get_descriptors": (C.c_int, [_P, _P]),
@@ -101,8 +103,7 @@ class Nep:
     """One context = one CUDA device + one stream (include/nep.h).  Method names are the C calls without `nep_`."""
 
     def __init__(self, n_species: int, rc_R: float, rc_A: float, n_max_R: int, n_max_A: int, basis_R: int, basis_A: int,
-                 l_max_3b: int = 4, l_max_4b: int = 2, l_max_5b: int = 1, neurons: int = 30, stream=None,
-                 use_torch_allocator: bool = True):
+                 l_max_3b: int = 4, l_max_4b: int = 2, l_max_5b: int = 1, neurons: int = 30, stream=None):
         import torch
         self._L = load_library()
         self._h = C.c_void_p(None)
@@ -117,7 +118,10 @@ class Nep:
 
         def _alloc(_user, nbytes):
             try:
-                t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda")
+                # allocate on the stream the library launches on: the caching allocator then reuses a freed block only
+                # in that stream's order, whatever torch's current stream is when the callback runs
+                with torch.cuda.stream(self.stream):
+                    t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda")
             except Exception:      # noqa: BLE001  (OOM -> NULL -> NEP_ENOMEM)
                 return None
             p = t.data_ptr()
@@ -130,8 +134,8 @@ class Nep:
             if t is not None:
                 self.bytes_allocated -= t.numel()
 
-        self._alloc_cb = ALLOC_FN(_alloc) if use_torch_allocator else C.cast(None, ALLOC_FN)
-        self._free_cb = FREE_FN(_free) if use_torch_allocator else C.cast(None, FREE_FN)
+        self._alloc_cb = ALLOC_FN(_alloc)
+        self._free_cb = FREE_FN(_free)
         h = C.c_void_p(None)
         rc = self._L.nep_create(C.byref(h), n_species, rc_R, rc_A, n_max_R, n_max_A, basis_R, basis_A, l_max_3b, l_max_4b,
                                 l_max_5b, neurons, self._alloc_cb, self._free_cb, None, C.c_void_p(stream.cuda_stream))
@@ -253,6 +257,17 @@ class Nep:
         self._ck(self._L.nep_get_scaler(self._h, _ptr(s)))
         return s
 
+    def compute_descriptor_range(self):
+        """(qmin, qmax), float64 [D] each: range of every descriptor component over this context's atoms."""
+        lo = np.zeros(self.D, np.float64); hi = np.zeros(self.D, np.float64)
+        self._ck(self._L.nep_compute_descriptor_range(self._h, _ptr(lo), _ptr(hi)))
+        self._batch_ids = np.arange(self.n_struct, dtype=np.int32)
+        return lo, hi
+
+    def set_scaler_from_range(self, qmin, qmax):
+        lo = _np(qmin, np.float64, (self.D,)); hi = _np(qmax, np.float64, (self.D,))
+        self._ck(self._L.nep_set_scaler_from_range(self._h, _ptr(lo), _ptr(hi)))
+
     # ---- step ----
     def set_batch(self, ids: Optional[Sequence[int]] = None):
         if ids is None:
@@ -317,7 +332,7 @@ class Nep:
                 if base <= ptr < base + t.numel():
                     off = ptr - base
                     return t[off:off + count * isz].view(dtype)
-            raise RuntimeError("device pointer is not inside a torch allocation (use_torch_allocator=False?)")
+            raise RuntimeError("device pointer is not inside an allocation of this context")
         return view(g.value, torch.float32, self.n_par), view(l.value, torch.float64, 4)
 
     def adam_step(self, lr: float, beta1: float = 0.9, beta2: float = 0.999, eps: float = 1e-8, variant: int = 0):

@@ -21,9 +21,7 @@ int fail(nep_ctx* c, int code, const std::string& msg)
 void* dev_alloc(nep_ctx* c, size_t bytes)
 {
     if (bytes == 0) bytes = 256;
-    void* p = nullptr;
-    if (c->alloc) p = c->alloc(c->user, bytes);
-    else if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+    void* p = c->alloc(c->user, bytes);   // the library never calls cudaMalloc: device memory is the caller's (include/nep.h)
     if (!p) { c->err = "device allocation of " + std::to_string(bytes) + " bytes failed"; return nullptr; }
     c->allocs.push_back(p);
     return p;
@@ -34,8 +32,7 @@ void dev_free(nep_ctx* c, void* p)
     if (!p) return;
     auto it = std::find(c->allocs.begin(), c->allocs.end(), p);
     if (it != c->allocs.end()) c->allocs.erase(it);
-    if (c->alloc) { if (c->free_) c->free_(c->user, p); }
-    else cudaFree(p);
+    c->free_(c->user, p);
 }
 
 void prof_begin(nep_ctx* c, const char* name)
@@ -133,12 +130,12 @@ int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max
     if (!(l_max_4b == 0 || l_max_4b == 2)) return fail(nullptr, NEP_EINVAL, "l_max_4b must be 0 or 2");
     if (!(l_max_5b == 0 || l_max_5b == 1)) return fail(nullptr, NEP_EINVAL, "l_max_5b must be 0 or 1");
     if (neurons < 1 || neurons > 512) return fail(nullptr, NEP_EINVAL, "neurons must be in 1..512");
-    if ((alloc == nullptr) != (free_ == nullptr)) return fail(nullptr, NEP_EINVAL, "alloc and free_ must both be given or both be NULL");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();
         return fail(nullptr, NEP_ECUDA, "no CUDA device: libnep_b200 has no CPU fallback");
     }
+    if (alloc == nullptr || free_ == nullptr) return fail(nullptr, NEP_EINVAL, "alloc and free_ are required: the library does not allocate device memory itself");
     nep_ctx* c = new (std::nothrow) nep_ctx();
     if (!c) return fail(nullptr, NEP_ENOMEM, "host allocation failed");
     c->rcR = rc_R; c->rcA = rc_A; c->n_max_R = n_max_R; c->n_max_A = n_max_A; c->basis_R = basis_R; c->basis_A = basis_A;
@@ -201,31 +198,33 @@ static void free_dataset(nep_ctx* c)
 static int upload_labels(nep_ctx* c, const double* E, const double* F, const double* W, const unsigned char* hv)
 {
     DataDev& d = c->d;
-    dev_free(c, (void*)d.Elab); dev_free(c, (void*)d.Flab); dev_free(c, (void*)d.Wlab); dev_free(c, (void*)d.hasv);
-    d.Elab = nullptr; d.Flab = nullptr; d.Wlab = nullptr; d.hasv = nullptr;
+    // validate before anything is released: a rejected call leaves the previous labels in place
     for (int64_t i = 0; i < c->S; ++i) if (!std::isfinite(E[i])) return fail(c, NEP_EINVAL, "non-finite energy label");
     for (int64_t i = 0; i < 3 * c->N; ++i) if (!std::isfinite(F[i])) return fail(c, NEP_EINVAL, "non-finite force label");
     for (int64_t i = 0; i < 9 * (int64_t)c->S; ++i) if (!std::isfinite(W[i])) return fail(c, NEP_EINVAL, "non-finite virial label");
-    std::vector<float> Fp((size_t)3 * c->NP, 0.0f), Wf((size_t)9 * c->S);
-    c->h_Flab.resize((size_t)3 * c->N);
-    for (int64_t i = 0; i < 3 * c->N; ++i) c->h_Flab[i] = (float)F[i];
+    std::vector<float> hF((size_t)3 * c->N), Fp((size_t)3 * c->NP, 0.0f), Wf((size_t)9 * c->S);
+    for (int64_t i = 0; i < 3 * c->N; ++i) hF[i] = (float)F[i];
     for (int s = 0; s < c->S; ++s)
         for (int i = 0; i < c->h_nat[s]; ++i)
             for (int k = 0; k < 3; ++k) {   // slice-blocked [slice][3][32], slot order
                 const int64_t p = c->h_pbase[s] + c->h_slot_of[c->h_aoff[s] + i];
-                Fp[(size_t)((p / WARP) * 3 + k) * WARP + p % WARP] = c->h_Flab[3 * (c->h_aoff[s] + i) + k];
+                Fp[(size_t)((p / WARP) * 3 + k) * WARP + p % WARP] = hF[3 * (c->h_aoff[s] + i) + k];
             }
     for (size_t i = 0; i < Wf.size(); ++i) Wf[i] = (float)W[i];
-    c->h_hasv.assign(c->S, 1);
-    if (hv) for (int s = 0; s < c->S; ++s) c->h_hasv[s] = hv[s] ? 1 : 0;
-    double* dE; float *dF, *dW; unsigned char* dh;
+    std::vector<unsigned char> hasv((size_t)c->S, 1);
+    if (hv) for (int s = 0; s < c->S; ++s) hasv[s] = hv[s] ? 1 : 0;
+    // upload into new buffers; the old ones are swapped out and released only after every copy has succeeded
+    double* dE = nullptr; float *dF = nullptr, *dW = nullptr; unsigned char* dh = nullptr;
     int rc;
-    if ((rc = upload<double>(c, dE, E, c->S))) return rc;
-    if ((rc = upload<float>(c, dF, Fp.data(), Fp.size()))) return rc;
-    if ((rc = upload<float>(c, dW, Wf.data(), Wf.size()))) return rc;
-    if ((rc = upload<unsigned char>(c, dh, c->h_hasv.data(), c->S))) return rc;
-    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    if ((rc = upload<double>(c, dE, E, c->S)) || (rc = upload<float>(c, dF, Fp.data(), Fp.size())) ||
+        (rc = upload<float>(c, dW, Wf.data(), Wf.size())) || (rc = upload<unsigned char>(c, dh, hasv.data(), c->S)) ||
+        (cudaStreamSynchronize(c->stream) != cudaSuccess && (rc = fail(c, NEP_ECUDA, "label upload failed")))) {
+        dev_free(c, dE); dev_free(c, dF); dev_free(c, dW); dev_free(c, dh);
+        return rc;
+    }
+    dev_free(c, (void*)d.Elab); dev_free(c, (void*)d.Flab); dev_free(c, (void*)d.Wlab); dev_free(c, (void*)d.hasv);
     d.Elab = dE; d.Flab = dF; d.Wlab = dW; d.hasv = dh;
+    c->h_Flab.swap(hF); c->h_hasv.swap(hasv);
     c->have_labels = true;
     c->grad_valid = false;
     return NEP_OK;
@@ -303,10 +302,13 @@ int nep_set_labels(nep_ctx* c, const double* E, const double* F, const double* W
     if (!c->have_data) return fail(c, NEP_ESTATE, "nep_set_labels before nep_load_structures");
     if (!E || !F || !W) return fail(c, NEP_EINVAL, "E, F and W are all required");
     int rc = upload_labels(c, E, F, W, has_virial);
-    if (rc == NEP_OK && c->have_nbrs) {   // Sv of the current batch depends on the mask
+    if (rc == NEP_OK && c->have_nbrs) {
+        // S_v of the current batch depends on the mask.  All three normalisers of Eqs. 5-7 go back to the counts of the
+        // local batch (as after nep_set_batch): a data-parallel caller gives the whole batch's counts again.
         int sv = 0;
         for (int sid : c->h_bsid) sv += c->h_hasv[sid];
-        c->b.Sv = sv; c->b.nrmV = (double)sv;
+        c->b.Sv = sv;
+        c->b.nrmS = (double)c->b.Sb; c->b.nrmN = (double)c->b.Nb; c->b.nrmV = (double)sv;
     }
     return rc;
 }
@@ -422,15 +424,52 @@ int nep_get_scaler(nep_ctx* c, double* s)
     for (int i = 0; i < c->m.D; ++i) s[i] = f[i];
     return NEP_OK;
 }
+// descriptors of every loaded atom at the current parameters, then their per-component minimum and maximum (device)
+static int descriptor_range_dev(nep_ctx* c, const char* who)
+{
+    if (!c->have_nbrs) return fail(c, NEP_ESTATE, std::string(who) + " before nep_build_neighbors");
+    if (!c->have_params) return fail(c, NEP_ESTATE, std::string(who) + " before nep_set_params");
+    int rc = nep_set_batch(c, 0, nullptr);
+    if (rc) return rc;
+    if (!c->qrange) { c->qrange = (float*)dev_alloc(c, 4 * 2 * (size_t)c->m.DP); if (!c->qrange) return NEP_ENOMEM; }
+    if ((rc = launch_forward(c, true))) return rc;
+    return launch_descriptor_range(c, c->qrange);
+}
 int nep_compute_scaler(nep_ctx* c)
 {
     CHECK_CTX(c);
-    if (!c->have_nbrs) return fail(c, NEP_ESTATE, "nep_compute_scaler before nep_build_neighbors");
-    if (!c->have_params) return fail(c, NEP_ESTATE, "nep_compute_scaler before nep_set_params");
-    int rc = nep_set_batch(c, 0, nullptr);
+    int rc = descriptor_range_dev(c, "nep_compute_scaler");
     if (rc) return rc;
-    if ((rc = launch_forward(c, true))) return rc;
-    if ((rc = launch_scaler_minmax(c, c->scaler))) return rc;
+    if ((rc = launch_scaler_from_range(c, c->qrange, c->scaler))) return rc;
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_scaler = true; c->forward_valid = c->grad_valid = false;
+    return NEP_OK;
+}
+int nep_compute_descriptor_range(nep_ctx* c, double* qmin, double* qmax)
+{
+    CHECK_CTX(c);
+    if (!qmin || !qmax) return fail(c, NEP_EINVAL, "qmin / qmax is NULL");
+    int rc = descriptor_range_dev(c, "nep_compute_descriptor_range");
+    if (rc) return rc;
+    std::vector<float> f(2 * (size_t)c->m.DP);
+    if ((rc = d2h(c, f.data(), c->qrange, 4 * f.size()))) return rc;
+    for (int v = 0; v < c->m.D; ++v) { qmin[v] = f[v]; qmax[v] = f[c->m.DP + v]; }
+    c->forward_valid = c->grad_valid = false;
+    return NEP_OK;
+}
+int nep_set_scaler_from_range(nep_ctx* c, const double* qmin, const double* qmax)
+{
+    CHECK_CTX(c);
+    if (!qmin || !qmax) return fail(c, NEP_EINVAL, "qmin / qmax is NULL");
+    std::vector<float> f(2 * (size_t)c->m.DP, 0.0f);
+    for (int v = 0; v < c->m.D; ++v) {
+        if (std::isnan(qmin[v]) || std::isnan(qmax[v])) return fail(c, NEP_EINVAL, "NaN in descriptor range");
+        f[v] = (float)qmin[v]; f[c->m.DP + v] = (float)qmax[v];
+    }
+    if (!c->qrange) { c->qrange = (float*)dev_alloc(c, 4 * f.size()); if (!c->qrange) return NEP_ENOMEM; }
+    int rc = h2d(c, c->qrange, f.data(), 4 * f.size());
+    if (rc) return rc;
+    if ((rc = launch_scaler_from_range(c, c->qrange, c->scaler))) return rc;
     NEP_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_scaler = true; c->forward_valid = c->grad_valid = false;
     return NEP_OK;
@@ -443,6 +482,8 @@ static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64
     if (NBP > c->cap_NBP) {
         void* olds[] = { b.q, b.Fp, b.S, b.Sd, b.qd, b.Qb, b.arow, b.Bd, b.F, b.u, b.Ei };
         for (void* p : olds) dev_free(c, p);
+        b.q = b.Fp = b.S = b.Sd = b.qd = b.Qb = b.arow = b.Bd = b.F = b.u = b.Ei = nullptr;   // a failed allocation below leaves no dangling pointer
+        c->cap_NBP = 0;
         size_t n = (size_t)NBP;
         ALLOC(c, b.q, float, n * m.D);   ALLOC(c, b.Fp, float, n * m.D);
         ALLOC(c, b.S, float, n * m.nA * 24); ALLOC(c, b.Sd, float, n * m.nA * 24);
@@ -453,6 +494,7 @@ static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64
     }
     if (tiles_m > c->cap_tiles_m) {
         dev_free(c, b.alist); dev_free(c, b.hbuf);
+        b.alist = nullptr; b.hbuf = nullptr; c->cap_tiles_m = 0;
         ALLOC(c, b.alist, int, tiles_m);
         ALLOC(c, b.hbuf, float, (size_t)tiles_m * m.HP);
         c->cap_tiles_m = tiles_m;
@@ -460,6 +502,7 @@ static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64
     if (Sb > c->cap_Sb) {
         void* olds[] = { b.Es, b.Ws, b.eps, b.G };
         for (void* p : olds) dev_free(c, p);
+        b.Es = nullptr; b.Ws = b.eps = b.G = nullptr; c->cap_Sb = 0;
         ALLOC(c, b.Es, double, Sb); ALLOC(c, b.Ws, float, 9 * (size_t)Sb); ALLOC(c, b.eps, float, Sb); ALLOC(c, b.G, float, 9 * (size_t)Sb);
         c->cap_Sb = Sb;
     }
@@ -513,8 +556,13 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
     int ntiles = 0;
     for (int t = 0; t < T; ++t) { b.tile_start[t] = ntiles; ntiles += (int)((tot[t] + TM - 1) / TM); }
     for (int t = T; t <= MAX_T; ++t) b.tile_start[t] = ntiles;
+    c->forward_valid = c->grad_valid = false;
     int rc = ensure_batch_capacity(c, std::max<int64_t>(nbs64 * WARP, WARP), std::max(Sb, 1), std::max(nbs, 1), std::max<int64_t>((int64_t)ntiles * TM, TM));
-    if (rc) return rc;
+    if (rc) {   // no batch is selected after a failed allocation: the step calls launch nothing
+        b.Sb = b.Sv = 0; b.Nb = 0; b.nbs = 0; b.NBP = 0; b.ntiles = 0;
+        c->h_bsid.clear(); c->h_bfoff.clear();
+        return rc;
+    }
     // tables, packed: binfo [nbs] int4 | bfoff [Sb] int64 | bsid [Sb] | bnat [Sb] | bsoff [Sb][T]
     char* h = (char*)c->h_stage;
     int4* binfo = (int4*)h;

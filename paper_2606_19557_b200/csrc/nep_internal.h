@@ -144,6 +144,7 @@ struct nep_ctx {
     void* h_stage = nullptr; size_t h_stage_bytes = 0; void* d_stage = nullptr; size_t d_stage_bytes = 0;
 
     float *theta = nullptr, *g = nullptr, *am = nullptr, *av = nullptr, *avmax = nullptr, *scaler = nullptr;
+    float* qrange = nullptr;   // [2][DP] per-component minimum and maximum of the descriptors (S0c)
     int64_t t_adam = 0;
     double lamE = 0, lamF = 0, lamV = 0;
 
@@ -170,10 +171,11 @@ void prof_end(nep_ctx* c);
 // ---- launchers (each returns NEP_OK or an error code with c->err set) ----
 int upload_slot_tables(nep_ctx* c);                            // nep_api.cu      : type_p, rank_p, orig_p, slot_of, force labels from h_slot_of
 int build_neighbors_dev(nep_ctx* c);                           // nep_neighbor.cu : S0a + S0b
-int launch_forward(nep_ctx* c, bool descriptors_only);         // nep_step.cu     : S1-S5
-int launch_loss_grad(nep_ctx* c);                              // nep_step.cu     : S6-S9
+int launch_forward(nep_ctx* c, bool descriptors_only);         // nep_misc.cu     : S1-S5
+int launch_loss_grad(nep_ctx* c);                              // nep_misc.cu     : S6-S9
 int launch_adam(nep_ctx* c, double lr, double b1, double b2, double eps, int variant);  // nep_adam.cu : S10
-int launch_scaler_minmax(nep_ctx* c, float* d_s);              // nep_misc.cu     : S0c (after a descriptors-only pass over all)
+int launch_descriptor_range(nep_ctx* c, float* d_rng);         // nep_misc.cu     : S0c min / max of q (after a descriptors-only pass over all)
+int launch_scaler_from_range(nep_ctx* c, const float* d_rng, float* d_s);   //         : S0c s = 1 / (max - min)
 int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW);  // nep_misc.cu: slice-blocked -> batch order
 int launch_gather_q(nep_ctx* c, float* dq);                    // [N_b][D]
 int launch_build_alist(nep_ctx* c);                            // nep_misc.cu     : type-sorted atom list of the batch

@@ -144,41 +144,56 @@ __global__ void k_gather_q(StepArgs a, float* q)
     const float* qp = sb_ptr(a.b.q, w, a.m.D, lane);
     for (int v = 0; v < a.m.D; ++v) q[o * a.m.D + v] = qp[(size_t)v * WARP];
 }
-// S0c (Eq. 2): one block per descriptor component: s = 1 / (max - min), degenerate range -> 1 (DESIGN G10)
-__global__ void __launch_bounds__(256) k_scaler_minmax(StepArgs a, float* s)
+// S0c (Eq. 2): one block per descriptor component: minimum and maximum over the atoms of the batch -> rng[v], rng[DP + v]
+// (no atoms: +inf, -inf, the neutral elements of a min / max exchange between data-parallel contexts)
+__global__ void __launch_bounds__(256) k_descriptor_range(StepArgs a, float* rng)
 {
     const int v = blockIdx.x;
-    float lo = INFINITY, hi = -INFINITY, am = 0.0f;
+    float lo = INFINITY, hi = -INFINITY;
     for (int64_t i = threadIdx.x; i < a.b.NBP; i += blockDim.x) {
         const int w = (int)(i >> 5), lane = (int)(i & 31);
         const int ds = a.b.binfo[w].x;
         if (a.d.type_p[(size_t)ds * WARP + lane] >= 0) {
             const float x = sb_ptr(a.b.q, w, a.m.D, lane)[(size_t)v * WARP];
-            lo = fminf(lo, x); hi = fmaxf(hi, x); am = fmaxf(am, fabsf(x));
+            lo = fminf(lo, x); hi = fmaxf(hi, x);
         }
     }
-    __shared__ float slo[256], shi[256], sam[256];
-    slo[threadIdx.x] = lo; shi[threadIdx.x] = hi; sam[threadIdx.x] = am;
+    __shared__ float slo[256], shi[256];
+    slo[threadIdx.x] = lo; shi[threadIdx.x] = hi;
     __syncthreads();
     for (int o = 128; o; o >>= 1) {
         if (threadIdx.x < o) {
             slo[threadIdx.x] = fminf(slo[threadIdx.x], slo[threadIdx.x + o]);
             shi[threadIdx.x] = fmaxf(shi[threadIdx.x], shi[threadIdx.x + o]);
-            sam[threadIdx.x] = fmaxf(sam[threadIdx.x], sam[threadIdx.x + o]);
         }
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        const float range = shi[0] - slo[0];
-        s[v] = (a.b.Nb > 0 && range > 1e-12f * fmaxf(1.0f, sam[0])) ? 1.0f / range : 1.0f;
+    if (threadIdx.x == 0) { rng[v] = slo[0]; rng[a.m.DP + v] = shi[0]; }
+}
+// s = 1 / (max - min) (Eq. 2).  A component without a range gets s = 1 (reading G10): "without a range" is a range below
+// the resolution of the arithmetic that produced q, here fp32 sums: 64 eps_fp32 max(1, max |q|) (the fp64 oracle: 1e-12).
+__global__ void k_scaler_from_range(int D, int DP, const float* __restrict__ rng, float* __restrict__ s)
+{
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= DP) return;
+    float out = 0.0f;
+    if (v < D) {
+        const float lo = rng[v], hi = rng[DP + v];
+        const float range = hi - lo, am = fmaxf(fabsf(lo), fabsf(hi));
+        out = (hi >= lo && isfinite(range) && range > 64.0f * 1.1920929e-7f * fmaxf(1.0f, am)) ? 1.0f / range : 1.0f;
     }
+    s[v] = out;
 }
 
-int launch_scaler_minmax(nep_ctx* c, float* d_s)
+int launch_descriptor_range(nep_ctx* c, float* d_rng)
 {
     StepArgs a = make_args(c);
-    NEP_CUDA(c, cudaMemsetAsync(d_s, 0, 4 * (size_t)c->m.DP, c->stream));
-    NEP_LAUNCH(c, "k_scaler_minmax", k_scaler_minmax, c->m.D, 256, 0, a, d_s);
+    NEP_LAUNCH(c, "k_descriptor_range", k_descriptor_range, c->m.D, 256, 0, a, d_rng);
+    return NEP_OK;
+}
+int launch_scaler_from_range(nep_ctx* c, const float* d_rng, float* d_s)
+{
+    NEP_LAUNCH(c, "k_scaler_from_range", k_scaler_from_range, (c->m.DP + 63) / 64, 64, 0, c->m.D, c->m.DP, d_rng, d_s);
     return NEP_OK;
 }
 

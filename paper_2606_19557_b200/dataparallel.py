@@ -11,8 +11,10 @@ periodic structure), so the units that shard are STRUCTURES:
                ONE exchange: all-reduce (sum) of g [N_par fp32] and of {L, dE, dF, dV} [4 fp64]
                (`allreduce_grad_loss`: NCCL on the GPU, gloo in the CPU tests); then every rank applies the same Adam update.
 
-The descriptor scaler (Eq. 2) is a min/max over every loaded atom: `allreduce_scaler` reduces the per-rank ranges.
-No arithmetic of the method lives here: the kernels are behind include/nep.h.
+The descriptor scaler (Eq. 2) is a range over every atom of the WHOLE set: every rank asks its context for the minimum and
+maximum of each component over its own atoms (nep_compute_descriptor_range), `allreduce_range` exchanges them (MIN / MAX),
+and every context forms the identical s = 1 / (max - min) itself (nep_set_scaler_from_range).
+No arithmetic of the method lives here: the kernels and the rule of Eq. 2 are behind include/nep.h.
 """
 from __future__ import annotations
 
@@ -74,65 +76,103 @@ def batch_normalisers(batch_ids: Sequence[int], n_atoms: Sequence[int], has_viri
     return int(len(b)), int(n[b].sum()), int(hv[b].sum())
 
 
-def allreduce_grad_loss(g, loss4, group=None):
-    """The step's one exchange: in-place sum over the ranks of the gradient and of the four loss terms."""
+def _on_stream(stream):
+    import contextlib
+    if stream is None:
+        return contextlib.nullcontext()
+    import torch
+    return torch.cuda.stream(stream)
+
+
+def allreduce_grad_loss(g, loss4, group=None, stream=None):
+    """The step's one exchange: in-place sum over the ranks of the gradient and of the four loss terms.
+    stream: the CUDA stream the context launches on (the collective is ordered after its kernels and before the Adam kernel)."""
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized():
-        dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)
-        dist.all_reduce(loss4, op=dist.ReduceOp.SUM, group=group)
+        with _on_stream(stream):
+            dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)
+            dist.all_reduce(loss4, op=dist.ReduceOp.SUM, group=group)
     return g, loss4
 
 
-def allreduce_scaler(qmin, qmax, group=None):
-    """Eq. 2 over every rank's atoms: s = 1 / (max - min) of the global ranges (degenerate range -> 1, DESIGN G10)."""
-    import torch
+def allreduce_range(qmin, qmax, group=None):
+    """Element-wise MIN of qmin and MAX of qmax over the ranks, in place (torch tensors on the backend's device).
+    +inf / -inf of a rank without atoms are the neutral elements."""
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
         dist.all_reduce(qmin, op=dist.ReduceOp.MIN, group=group)
         dist.all_reduce(qmax, op=dist.ReduceOp.MAX, group=group)
-    rng = qmax - qmin
-    big = torch.maximum(qmax.abs(), qmin.abs()).clamp_min(1.0)
-    return torch.where(rng > 1e-12 * big, 1.0 / rng, torch.ones_like(rng))
+    return qmin, qmax
 
 
 class DataParallelNep:
-    """A `Nep` context holding this rank's share of a structure set, driven with GLOBAL structure ids."""
+    """A `Nep` context holding this rank's share of a structure set, driven with GLOBAL structure ids.
 
-    def __init__(self, model, structures, rank: int, world: int, group=None, **kw):
-        from .binding import Nep
+    nep_factory(model, **kw) builds the context (default: binding.Nep.from_model); the CPU tests pass a stand-in."""
+
+    def __init__(self, model, structures, rank: int, world: int, group=None, work=None, nep_factory=None, **kw):
         self.group = group
         self.n_atoms = np.asarray(structures.n_atoms, dtype=np.int64)
-        self.shard = Shard.make(self.n_atoms, rank, world)
+        self.shard = Shard.make(self.n_atoms, rank, world, work)
         self.has_virial = np.ones(len(self.n_atoms), dtype=np.int64)
-        self.nep = Nep.from_model(model, **kw)
+        if nep_factory is None:
+            from .binding import Nep
+            nep_factory = Nep.from_model
+        self.nep = nep_factory(model, **kw)
         self.structures = structures
         self._whole = (0, 0, 0)
 
+    def _local_rows(self):
+        off = np.concatenate([[0], np.cumsum(self.n_atoms)])
+        ids = self.shard.global_ids
+        return np.concatenate([np.arange(off[s], off[s + 1]) for s in ids]) if len(ids) else np.zeros(0, np.int64)
+
     def load(self, E=None, F=None, W=None, has_virial=None):
-        """Loads this rank's structures (labels optional, global arrays in the caller's order)."""
-        st = self.structures
-        sub = st.subset(self.shard.global_ids)
+        """Loads this rank's structures (labels optional, global arrays in the caller's order) and builds its lists."""
+        sub = self.structures.subset(self.shard.global_ids)
         if has_virial is not None:
             self.has_virial = np.asarray(has_virial, dtype=np.int64)
         if E is None:
             self.nep.load_structure_set(sub)
         else:
-            off = np.concatenate([[0], np.cumsum(self.n_atoms)])
-            rows = np.concatenate([np.arange(off[s], off[s + 1]) for s in self.shard.global_ids]) if len(self.shard.global_ids) else np.zeros(0, np.int64)
-            hv = None if has_virial is None else np.asarray(has_virial, dtype=np.uint8)[self.shard.global_ids]
-            self.nep.load_structure_set(sub, np.asarray(E)[self.shard.global_ids], np.asarray(F)[rows], np.asarray(W)[self.shard.global_ids], hv)
+            ids = self.shard.global_ids
+            hv = None if has_virial is None else np.asarray(has_virial, dtype=np.uint8)[ids]
+            self.nep.load_structure_set(sub, np.asarray(E)[ids], np.asarray(F)[self._local_rows()], np.asarray(W)[ids], hv)
         self.nep.build_neighbors()
+
+    def set_labels(self, E, F, W, has_virial=None):
+        """Attaches labels given for the WHOLE set (caller's order) to this rank's structures."""
+        ids = self.shard.global_ids
+        if has_virial is not None:
+            self.has_virial = np.asarray(has_virial, dtype=np.int64)
+        hv = None if has_virial is None else np.asarray(has_virial, dtype=np.uint8)[ids]
+        self.nep.set_labels(np.asarray(E)[ids], np.asarray(F)[self._local_rows()], np.asarray(W)[ids], hv)
+
+    def compute_scaler(self):
+        """Eq. 2 over the atoms of every rank: local ranges -> MIN / MAX all-reduce -> the same scaler in every context."""
+        import torch
+        import torch.distributed as dist
+        lo, hi = self.nep.compute_descriptor_range()
+        dev = "cpu"
+        if dist.is_available() and dist.is_initialized() and dist.get_backend(self.group) == "nccl":
+            dev = "cuda"
+        tlo, thi = torch.from_numpy(np.array(lo)).to(dev), torch.from_numpy(np.array(hi)).to(dev)
+        allreduce_range(tlo, thi, self.group)
+        self.nep.set_scaler_from_range(tlo.cpu().numpy(), thi.cpu().numpy())
 
     def set_batch(self, batch_ids: Sequence[int]):
         self.nep.set_batch(self.shard.local_batch(batch_ids))
         self._whole = batch_normalisers(batch_ids, self.n_atoms, self.has_virial)
         self.nep.set_batch_normalisers(*self._whole)
 
+    def local_batch_shape(self):
+        return self.nep.batch_shape()
+
     def step(self, lam, lr: float, fetch_loss: bool = False):
         """One training step on the current batch: forward, loss + gradient, the all-reduce, Adam."""
         self.nep.forward_device()
         self.nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
         g, l4 = self.nep.grad_loss_tensors()
-        allreduce_grad_loss(g, l4, self.group)
+        allreduce_grad_loss(g, l4, self.group, getattr(self.nep, "stream", None))
         self.nep.adam_step(lr)
         return l4.cpu().numpy() if fetch_loss else None

@@ -78,6 +78,69 @@ def _rank_main(rank, world, port, out):
         dist.destroy_process_group()
 
 
+def _rank_dp_nep(rank, world, port, out):
+    """DataParallelNep end to end on the CPU (oracle-backed stand-in context): the two ranks hold DIFFERENT structures."""
+    import torch.distributed as dist
+    from tests._oracle_nep import OracleNep
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        O.set_num_threads(1)
+        w = wl.tiny_workload(11, n_species=2, sizes=(5, 9, 3, 7, 6, 4), box=(3.4, 4.3, 3.1, 3.9, 3.6, 4.0))
+        prob = H.make_problem(w)
+        st = w.structures
+        hv = np.array([1, 0, 1, 1, 1, 0], np.uint8)
+        d = dp.DataParallelNep(w.model, st, rank, world, nep_factory=OracleNep.from_model)
+        d.load(prob.E, prob.F, prob.W, hv)
+        d.nep.set_params(prob.theta)
+        lo, hi = d.nep.compute_descriptor_range()              # this rank's own atoms only
+        d.compute_scaler()                                     # Eq. 2 over the union
+        s = d.nep.get_scaler()
+        batch = np.array([4, 0, 5, 2, 1], np.int32)
+        lam = (1.0, 2.0, 3.0)
+        d.set_batch(batch)
+        l4 = d.step(lam, 1e-2, fetch_loss=True)
+        out.put((rank, s, lo, hi, l4, d.nep.get_params(), [int(x) for x in d.shard.global_ids], d.local_batch_shape()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_dataparallel_nep_scaler_and_step_gloo_world2():
+    """Eq. 2 is over every atom of the set: two ranks with different structures (and different local ranges) must end with
+    the identical scaler, equal to the oracle's over the union; one DataParallelNep.step then lands both on the parameters
+    of the oracle's whole-batch step."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rank_dp_nep, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted((out.get(timeout=240) for _ in range(2)), key=lambda r: r[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, s0, lo0, hi0, l40, th0, ids0, shp0), (_, s1, lo1, hi1, l41, th1, ids1, shp1) = res
+    assert sorted(ids0 + ids1) == list(range(6)) and ids0 and ids1 and not set(ids0) & set(ids1)
+    assert not np.allclose(lo0, lo1) and not np.allclose(hi0, hi1)            # the local ranges differ ...
+    assert np.array_equal(s0, s1)                                             # ... the scaler does not
+    w = wl.tiny_workload(11, n_species=2, sizes=(5, 9, 3, 7, 6, 4), box=(3.4, 4.3, 3.1, 3.9, 3.6, 4.0))
+    prob = H.make_problem(w)
+    s_union = O.scaler(O.descriptors(prob.data, prob.theta))                   # Eq. 2 over the union, at the same theta
+    assert np.allclose(s0, s_union, rtol=1e-12)
+    assert not np.allclose(1.0 / (hi0 - lo0), s_union, rtol=1e-3)             # a rank-local scaler would have been wrong
+    hv = np.array([1, 0, 1, 1, 1, 0], np.uint8)
+    prob.data.set_labels(prob.E, prob.F, prob.W, hv)
+    batch = [4, 0, 5, 2, 1]
+    l4w, gw = O.loss_grad(prob.data, prob.theta, s_union, (1.0, 2.0, 3.0), batch=batch)
+    assert np.allclose(l40, l4w, rtol=1e-10) and np.array_equal(l40, l41)
+    th = prob.theta.copy(); n = th.size
+    O.adam_step(th, gw.astype(np.float32).astype(np.float64), np.zeros(n), np.zeros(n), np.zeros(n), 0, 1e-2)
+    assert np.array_equal(th0, th1)                                           # identical updates, no parameter broadcast
+    assert np.max(np.abs(th0 - th)) < 2e-6
+    assert shp0[0] + shp1[0] == 5
+
+
 def test_shares_add_up_gloo_world2():
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")

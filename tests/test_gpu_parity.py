@@ -156,6 +156,35 @@ def test_load_rejects_bad_input():
         nep.build_neighbors()
 
 
+def test_rejected_labels_leave_the_old_ones_in_place():
+    """nep_set_labels validates before it releases anything: after a rejected call (NaN label) the previous labels still
+    serve nep_loss_grad, with the values they had."""
+    from paper_2606_19557_b200.binding import NepError, NEP_EINVAL
+    prob = _prob("tiny_T2")
+    with H.make_gpu(prob) as nep:
+        nep.forward(want=())
+        l4 = nep.loss_grad(1.0, 2.0, 3.0)
+        for which in range(3):
+            E, F, W = prob.E.copy(), prob.F.copy(), prob.W.copy()
+            (E, F, W)[which].flat[0] = np.nan if which != 1 else np.inf
+            with pytest.raises(NepError) as e:
+                nep.set_labels(E, F, W)
+            assert e.value.code == NEP_EINVAL
+        nep.forward(want=())
+        assert np.array_equal(nep.loss_grad(1.0, 2.0, 3.0), l4)
+
+
+def test_null_allocator_is_refused():
+    """include/nep.h: the library never calls cudaMalloc; a context without allocator callbacks is NEP_EINVAL."""
+    import ctypes
+    from paper_2606_19557_b200 import binding
+    L = binding.load_library()
+    h = ctypes.c_void_p(None)
+    rc = L.nep_create(ctypes.byref(h), 1, 5.0, 4.0, 4, 4, 8, 8, 4, 2, 1, 30, ctypes.cast(None, binding.ALLOC_FN),
+                      ctypes.cast(None, binding.FREE_FN), None, None)
+    assert rc == binding.NEP_EINVAL and b"alloc" in L.nep_last_error(None) and not h.value
+
+
 def test_virial_mask():
     prob = _prob("tiny_T3_ragged")
     hv = np.array([1, 0, 1], np.uint8)
@@ -178,6 +207,72 @@ def test_compute_scaler_matches_definition(name):
     with H.make_gpu(prob, scaler="compute") as nep:
         s = nep.get_scaler()
     assert np.allclose(s, prob.scaler, rtol=2e-5), np.max(np.abs(s / prob.scaler - 1))
+
+
+def test_scaler_of_a_perfect_lattice():
+    """Reading G10: a component that is the same for every atom has no range and gets s = 1.  On a perfect lattice every
+    component is constant; in fp32 its "range" is summation noise (~1e-7 |q|), which must not be inverted into s ~ 1e7."""
+    pos, cell = wl._lattice("bcc", 3.16, (4, 4, 4))
+    st = wl.StructureSet(np.array([len(pos)], np.int32), wl._wrap(pos, cell), cell.reshape(1, 9), np.zeros(len(pos), np.int32), ["bcc"])
+    w = wl.make_config(2, n_struct=1)
+    import dataclasses
+    w = dataclasses.replace(w, structures=st)
+    from paper_2606_19557_b200.binding import Nep
+    th = wl.ParamDraw(w.model, w.seeds["student"]).coefficients()
+    q = O.descriptors(O.OracleData(w.model, st), th)
+    assert np.array_equal(O.scaler(q), np.ones(w.model.D))               # the oracle: every range is below 1e-12 max(1, |q|)
+    with Nep.from_model(w.model) as nep:
+        nep.load_structure_set(st)
+        nep.build_neighbors()
+        nep.set_params(th.astype(np.float32))
+        nep.compute_scaler()
+        assert np.array_equal(nep.get_scaler(), np.ones(w.model.D))
+        lo, hi = nep.compute_descriptor_range()
+        assert np.all(hi - lo <= 1e-5 * np.maximum(1.0, np.abs(hi)))     # fp32 noise only
+        assert np.allclose(0.5 * (lo + hi), q.mean(0), rtol=1e-5, atol=1e-6)
+
+
+def test_descriptor_range_of_two_contexts_gives_the_scaler_of_the_union():
+    """Eq. 2 is over every atom of the set.  Two contexts hold different structures: their ranges, reduced element-wise
+    (the MIN / MAX all-reduce of dataparallel.DataParallelNep.compute_scaler), give each of them the scaler that one context
+    holding everything computes, which is the oracle's."""
+    from paper_2606_19557_b200 import dataparallel as dp
+    from paper_2606_19557_b200.binding import Nep
+    prob = _prob("cfg3")
+    w = prob.workload; st = w.structures
+    s_union = O.scaler(O.descriptors(prob.data, prob.theta))
+    los, his, ctxs = [], [], []
+    try:
+        for rank in range(2):
+            ids = dp.Shard.make(st.n_atoms, rank, 2).global_ids
+            nep = Nep.from_model(w.model)
+            ctxs.append(nep)
+            nep.load_structure_set(st.subset(ids))
+            nep.build_neighbors()
+            nep.set_params(prob.theta.astype(np.float32))
+            lo, hi = nep.compute_descriptor_range()
+            los.append(lo); his.append(hi)
+        assert not np.allclose(los[0], los[1]) and not np.allclose(his[0], his[1])
+        lo, hi = np.minimum(*los), np.maximum(*his)
+        for nep in ctxs:
+            nep.set_scaler_from_range(lo, hi)
+        s0, s1 = ctxs[0].get_scaler(), ctxs[1].get_scaler()
+        assert np.array_equal(s0, s1)
+        assert np.allclose(s0, s_union, rtol=2e-5), np.max(np.abs(s0 / s_union - 1))
+        with H.make_gpu(prob, labels=False, scaler="compute") as whole:
+            assert np.allclose(s0, whole.get_scaler(), rtol=1e-6)
+        # an empty context reports the neutral elements and takes the reduced range like every other
+        with Nep.from_model(w.model) as empty:
+            empty.load_structure_set(st.subset([]))
+            empty.build_neighbors()
+            empty.set_params(prob.theta.astype(np.float32))
+            elo, ehi = empty.compute_descriptor_range()
+            assert np.all(np.isposinf(elo)) and np.all(np.isneginf(ehi))
+            empty.set_scaler_from_range(lo, hi)
+            assert np.array_equal(empty.get_scaler(), s0)
+    finally:
+        for nep in ctxs:
+            nep.destroy()
 
 
 @pytest.mark.parametrize("variant", [0, 1])
