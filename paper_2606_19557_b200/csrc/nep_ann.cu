@@ -27,7 +27,6 @@ struct AnnLay {
     int TM, LD, DP8, HP8, HP32, TK, TKP, nR8;
     int W0m, W0t, b0, w1, sc, cRs, cRt, Qs, QDs, Gs, Es, Bs, BDs, FPs, ibs, aux, red, total;   // float offsets
 };
-__host__ __device__ inline int rup(int x, int m) { return (x + m - 1) / m * m; }
 __host__ __device__ inline AnnLay ann_layout(const ModelDev& m, int TM, bool bwd)
 {
     AnnLay l;
@@ -174,12 +173,6 @@ __device__ __forceinline__ void for_chunks(int N, F&& f)
     }
 }
 
-__device__ __forceinline__ int tile_type(const BatchDev& b, int tile, int T)
-{
-    int t = 0;
-    while (t + 1 < T && tile >= b.tile_start[t + 1]) ++t;
-    return t;
-}
 
 // weights of species t into shared memory, zero padded and with the scaler folded in:
 // W0m[mu][v] = W0t[v][mu] = w0[mu][v] s_v;  b0, w1, scaler
@@ -259,7 +252,7 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_fwd(StepArgs a)
         for (int v = m.D + rg; v < l.DP8; v += RG) sm[l.Qs + v * LD + am] = 0.0f;
         if (rg == 0) ibs[am] = ib;
     }
-    const int t = tile_type(a.b, tile, m.T);
+    const int t = tile_type_of(a.b, tile, m.T);
     if (t != cur_t) {
         cur_t = t;
         ann_load_weights(a, l, sm, t, true);
@@ -390,7 +383,7 @@ __global__ void __launch_bounds__(8 * TM / AT) k_ann_bwd(StepArgs a)
         if (rg == 0) { sm[l.aux + am] = epsi; ibs[am] = ib; }
         for (int v = m.D + rg; v < l.DP8; v += RG) { sm[l.Qs + v * LD + am] = 0.0f; sm[l.QDs + v * LD + am] = 0.0f; }
     }
-    const int t = tile_type(a.b, tile, m.T);
+    const int t = tile_type_of(a.b, tile, m.T);
     if (t != cur_t) {
         cur_t = t;
         ann_load_weights(a, l, sm, t, false);
@@ -532,6 +525,7 @@ constexpr int ANN_AT = 4;   // atoms per thread: 256 threads per 128-atom tile
 
 int ann_tile_m(const nep_ctx* c)
 {
+    if (c->ann_tc) return 128;
     // 128-atom tiles while two blocks of the larger (backward) kernel fit in one SM's shared memory, else 64
     const size_t bytes128 = 4 * (size_t)ann_layout(c->m, 128, true).total;
     return bytes128 <= 110 * 1024 ? 128 : 64;
@@ -561,7 +555,15 @@ static int launch_ann_t(nep_ctx* c, const StepArgs& a, bool bwd)
     }
     return NEP_OK;
 }
-int launch_ann_fwd(nep_ctx* c, const StepArgs& a) { return c->b.tile_m == 128 ? launch_ann_t<128>(c, a, false) : launch_ann_t<64>(c, a, false); }
-int launch_ann_bwd(nep_ctx* c, const StepArgs& a) { return c->b.tile_m == 128 ? launch_ann_t<128>(c, a, true) : launch_ann_t<64>(c, a, true); }
+int launch_ann_fwd(nep_ctx* c, const StepArgs& a)
+{
+    if (c->ann_tc) return launch_ann_fwd_tc(c, a);
+    return c->b.tile_m == 128 ? launch_ann_t<128>(c, a, false) : launch_ann_t<64>(c, a, false);
+}
+int launch_ann_bwd(nep_ctx* c, const StepArgs& a)
+{
+    if (c->ann_tc) return launch_ann_bwd_tc(c, a);
+    return c->b.tile_m == 128 ? launch_ann_t<128>(c, a, true) : launch_ann_t<64>(c, a, true);
+}
 
 }  // namespace nep

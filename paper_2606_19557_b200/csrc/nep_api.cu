@@ -1,12 +1,13 @@
 // nep_api.cu -- C ABI entry points of libnep_b200 (include/nep.h): argument checks, state machine,
 // host<->device marshalling.  All arithmetic of the step lives in the kernels of the other .cu files.
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
 #include <new>
 
-#include "nep_internal.h"
+#include "nep_kernels.cuh"
 
 static thread_local std::string g_create_error;
 
@@ -152,6 +153,10 @@ int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&c->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    {   // network kernels: tensor-core tiles when they fit; NEP_ANN_FFMA=1 selects the FFMA tiles (measurement aid)
+        const char* e = getenv("NEP_ANN_FFMA");
+        c->ann_tc = !(e && e[0] == '1') && ann_tc_fits(c, false) && ann_tc_fits(c, true);
+    }
     size_t np = (size_t)m.npar;
     c->theta = (float*)dev_alloc(c, 4 * np); c->g = (float*)dev_alloc(c, 4 * np); c->am = (float*)dev_alloc(c, 4 * np);
     c->av = (float*)dev_alloc(c, 4 * np); c->avmax = (float*)dev_alloc(c, 4 * np); c->scaler = (float*)dev_alloc(c, 4 * (size_t)m.DP);

@@ -120,6 +120,7 @@ struct nep_ctx {
     std::string err;
     std::vector<void*> allocs;
     int sm_count; int max_smem_optin;
+    bool ann_tc = false;   // network kernels on tcgen05 (nep_ann_tc.cu) instead of the FFMA tiles (nep_ann.cu)
 
     // host copies of the data set
     int S = 0; int64_t N = 0, NP = 0; int nslices = 0;

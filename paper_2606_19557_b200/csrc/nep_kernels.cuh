@@ -29,6 +29,17 @@ struct Lane {
     unsigned ib;   // batch-padded atom index w*32 + lane
 };
 
+__host__ __device__ inline int rup(int x, int m) { return (x + m - 1) / m * m; }
+
+// species of a network tile (tiles are sorted by species; b.tile_start[t] = first tile of species t)
+__device__ __forceinline__ int tile_type_of(const BatchDev& b, int tile, int T)
+{
+    int t = 0;
+#pragma unroll 1
+    while (t + 1 < T && tile >= b.tile_start[t + 1]) ++t;
+    return t;
+}
+
 // false if the warp is beyond the batch (whole warp returns together)
 __device__ __forceinline__ bool lane_init(const StepArgs& a, Lane& L)
 {
@@ -348,5 +359,9 @@ int launch_rad_tangent(nep_ctx* c, const StepArgs& a);
 int launch_ann_fwd(nep_ctx* c, const StepArgs& a);
 int launch_ann_bwd(nep_ctx* c, const StepArgs& a);
 int launch_loss(nep_ctx* c, const StepArgs& a);
+// tensor-core network kernels (nep_ann_tc.cu); ann_tc_fits: the model's tiles fit in shared memory and TMEM
+bool ann_tc_fits(const nep_ctx* c, bool bwd);
+int launch_ann_fwd_tc(nep_ctx* c, const StepArgs& a);
+int launch_ann_bwd_tc(nep_ctx* c, const StepArgs& a);
 
 }  // namespace nep
