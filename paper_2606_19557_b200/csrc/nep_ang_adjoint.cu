@@ -226,6 +226,162 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Several species, second design.  One warp per block, blockIdx.z = pass.  A lane's accumulators are never cleared: when its
+// run of neighbour type t ends it stores a SNAPSHOT of them (12 x 128-bit stores into its own row of a lane-major table
+// snap[lane][t][n k], row stride an odd number of 16-byte units: conflict free); types the lane does not meet get the snapshot
+// of the type before them, so that the sum over the pairs with neighbour type t is snap[t] - snap[t - 1] for every lane.
+// After the sweep the lanes of one centre type are a contiguous range (slot order of a slice): thread r sums column
+// r = (t, n, k) over that range and issues one RED per (t_i, t_j, n, k).
+// ------------------------------------------------------------------------------------------------
+template <int NCH, int K>
+__global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a)
+{
+    extern __shared__ __align__(16) float smem[];
+    const ModelDev& m = a.m;
+    constexpr int NK = NCH * K, NKP = (NK + 3) & ~3, KH = (K + 1) / 2;
+    const int T = m.T;
+    const int LS = (T * NKP) + (((T * NKP) >> 2) & 1 ? 0 : 4);          // lane stride (words): LS / 4 odd
+    float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;      // SWEEP_STAGES cells per thread, WARP apart
+    float* tab = smem + (WARP * 4 * SWEEP_STAGES);
+    const int n0 = blockIdx.y * NCH;
+    const int lane = threadIdx.x;
+    Lane L;
+    lane_init_slice(a, L, (int)blockIdx.x);
+    float2 acc2[NCH][KH];
+#pragma unroll
+    for (int n = 0; n < NCH; ++n)
+#pragma unroll
+        for (int k = 0; k < KH; ++k) acc2[n][k] = make_float2(0.0f, 0.0f);
+    auto accv = [&](int e) -> float { const int n = e / K, k = e - n * K; return e < NK ? ((k & 1) ? acc2[n][k >> 1].y : acc2[n][k >> 1].x) : 0.0f; };
+    float* mine = tab + (size_t)lane * LS;
+    int cur = 0;
+    auto snapshot_to = [&](int tj) {      // rows cur .. tj - 1 <- the accumulators as they are
+        while (cur < tj) {
+            float4* dst = reinterpret_cast<float4*>(mine + cur * NKP);
+#pragma unroll
+            for (int i = 0; i < NKP / 4; ++i) dst[i] = make_float4(accv(4 * i), accv(4 * i + 1), accv(4 * i + 2), accv(4 * i + 3));
+            ++cur;
+        }
+    };
+    if (L.ti >= 0) {
+        const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+        const float rcinv = m.rcinvA;
+        float2 X2[NCH][NL / 2];
+        if (blockIdx.z == 0) {
+            {
+                float X[NCH][NL];
+                const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
+                const float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
+                const float* Qbp = sb_ptr(a.b.Qb, L.w, m.D, L.lane);
+                const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
+#pragma unroll
+                for (int n = 0; n < NCH; ++n) {
+                    if (n0 + n < m.nA) {
+                        float S[NL], Sd[NL], cq[6], cf[6];
+                        const size_t o = (size_t)(n0 + n) * NL * WARP;
+#pragma unroll
+                        for (int l = 0; l < NL; ++l) { S[l] = Sp[o + l * WARP]; Sd[l] = Sdp[o + l * WARP]; }
+                        load_inv_coef(m, Qbp, n0 + n, cq);
+                        load_inv_coef(m, Fpp, n0 + n, cf);
+                        inv_adjoint(S, cq, X[n]);
+                        inv_hessian_action(S, Sd, cf, X[n]);
+                    } else {
+#pragma unroll
+                        for (int l = 0; l < NL; ++l) X[n][l] = 0.0f;
+                    }
+                    pack24(X[n], X2[n]);
+                }
+            }
+            sweep_pairs_tb<WARP>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
+                const PairGeo p = pair_geo(rc4);
+                snapshot_to(p.tj);
+                float b[NL], al[NCH];
+                float2 b2[NL / 2];
+                harm24(harm_z(p.z), harm_xy(p.x, p.y), b);
+                pack24(b, b2);
+#pragma unroll
+                for (int n = 0; n < NCH; ++n) {
+                    float2 s1 = make_float2(0.0f, 0.0f);
+#pragma unroll
+                    for (int l = 0; l < NL / 2; ++l) s1 = __ffma2_rn(X2[n][l], b2[l], s1);
+                    al[n] = s1.x + s1.y;
+                }
+                float fv[2 * KH];
+                fv[2 * KH - 1] = 0.0f;
+                cheb_basis<K, false>(p.r, rcinv, [&](int k, float fk, float) { fv[k] = fk; });
+#pragma unroll
+                for (int n = 0; n < NCH; ++n) {
+                    const float2 aa = dup2(al[n]);
+#pragma unroll
+                    for (int k = 0; k < KH; ++k) acc2[n][k] = __ffma2_rn(aa, make_float2(fv[2 * k], fv[2 * k + 1]), acc2[n][k]);
+                }
+            });
+        } else {
+            {
+                float X[NCH][NL];
+                load_EdS<NCH>(a, L, n0, X);
+#pragma unroll
+                for (int n = 0; n < NCH; ++n) pack24(X[n], X2[n]);
+            }
+            float G[9];
+#pragma unroll
+            for (int k = 0; k < 9; ++k) G[k] = __ldg(a.b.G + 9 * L.sb + k);
+            const float* ui = sb_ptr(a.b.u, L.w, 3, L.lane);
+            const float uix = ui[0], uiy = ui[WARP], uiz = ui[2 * WARP];
+            const float* ub = a.b.u;
+            const int bbase = L.bbase;
+            sweep_pairs_tb<WARP>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
+                const PairGeo p = pair_geo(rc4);
+                snapshot_to(p.tj);
+                const Tangent Tg = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
+                float b[NL], bd[NL], be[NCH], de[NCH];
+                float2 b2[NL / 2], bd2[NL / 2];
+                const HarmZ hz = harm_z(p.z);
+                const HarmXY hxy = harm_xy(p.x, p.y);
+                harm24(hz, hxy, b);
+                harm24_tangent(hz, hxy, Tg.rx, Tg.ry, Tg.rz, bd);
+                pack24(b, b2); pack24(bd, bd2);
+#pragma unroll
+                for (int n = 0; n < NCH; ++n) {
+                    float2 s1 = make_float2(0.0f, 0.0f), s2 = make_float2(0.0f, 0.0f);
+#pragma unroll
+                    for (int l = 0; l < NL / 2; ++l) { s1 = __ffma2_rn(X2[n][l], b2[l], s1); s2 = __ffma2_rn(X2[n][l], bd2[l], s2); }
+                    be[n] = (s1.x + s1.y) * Tg.t; de[n] = s2.x + s2.y;
+                }
+                float fv[2 * KH], dfv[2 * KH];
+                fv[2 * KH - 1] = 0.0f; dfv[2 * KH - 1] = 0.0f;
+                cheb_basis<K, true>(p.r, rcinv, [&](int k, float fk, float dfk) { fv[k] = fk; dfv[k] = dfk; });
+#pragma unroll
+                for (int n = 0; n < NCH; ++n) {
+                    const float2 dd = dup2(de[n]), bb = dup2(be[n]);
+#pragma unroll
+                    for (int k = 0; k < KH; ++k)
+                        acc2[n][k] = __ffma2_rn(dd, make_float2(fv[2 * k], fv[2 * k + 1]), __ffma2_rn(bb, make_float2(dfv[2 * k], dfv[2 * k + 1]), acc2[n][k]));
+                }
+            });
+        }
+    }
+    snapshot_to(T);                       // the run in progress and the types after it (a lane without pairs: zeros everywhere)
+    __syncwarp();
+    // column sums per centre type: the lanes of one type are a contiguous range
+    const int rows = T * NKP;
+    const size_t tstep = (size_t)T * m.nA * m.KA;
+    for (int ti = 0; ti < T; ++ti) {
+        const unsigned bm = __ballot_sync(0xffffffffu, L.ti == ti);
+        if (bm == 0u) continue;
+        const int c0 = __ffs(bm) - 1, c1 = c0 + __popc(bm);
+        for (int r = lane; r < rows; r += WARP) {
+            const int tj = r / NKP, e = r - tj * NKP, n = e / K, k = e - n * K;
+            if (!(e < NK && k < m.KA && n0 + n < m.nA)) continue;
+            float v = 0.0f;
+            if (tj > 0) { for (int c = c0; c < c1; ++c) v += tab[(size_t)c * LS + r] - tab[(size_t)c * LS + r - NKP]; }
+            else { for (int c = c0; c < c1; ++c) v += tab[(size_t)c * LS + r]; }
+            if (v != 0.0f) atomicAdd(a.g + m.o_cA + ((size_t)tj * m.nA + n0 + n) * m.KA + k + ti * tstep, v);
+        }
+    }
+}
+
 int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
 {
     const ModelDev& m = c->m;
@@ -237,15 +393,13 @@ int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
             const size_t smem = (size_t)SWEEP_SMEM_BYTES + 4 * (size_t)nw * NK;
             NEP_LAUNCH(c, "k_ang_adjoint", (k_ang_adjoint<NCH, K, false>), dim3((unsigned)((c->b.nbs + nw - 1) / nw), a.nchunks), nw * WARP, smem, a);
         } else {
-            auto bytes = [&](int nw) { return (size_t)SWEEP_SMEM_BYTES + 4 * (size_t)nw * ((size_t)m.T * NK * ADJ_TST + m.T); };
-            // one warp per block: the per-lane table columns of a warp take up to 30 KB, and one-warp blocks fill the SM's
-            // shared memory in the finest steps (config 4: 7 instead of 6 warps per SM, 626 -> 597 us)
-            const int nw = 1;
-            const size_t smem = bytes(nw);
+            constexpr int NKP = (NK + 3) & ~3;
+            const int LS = (m.T * NKP) + ((((m.T * NKP) >> 2) & 1) ? 0 : 4);
+            const size_t smem = (size_t)WARP * 16 * SWEEP_STAGES + 4 * (size_t)WARP * LS;
             if (smem > (size_t)c->max_smem_optin) return fail(c, NEP_ECAPACITY, "angular coefficient tables do not fit in shared memory");
-            auto kern = k_ang_adjoint<NCH, K, true>;
+            auto kern = k_ang_adjoint_ms<NCH, K>;
             if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            NEP_LAUNCH(c, "k_ang_adjoint", kern, dim3((unsigned)((c->b.nbs + nw - 1) / nw), a.nchunks, 2), nw * WARP, smem, a);
+            NEP_LAUNCH(c, "k_ang_adjoint", kern, dim3((unsigned)c->b.nbs, a.nchunks, 2), WARP, smem, a);
         }
     });
     return NEP_OK;

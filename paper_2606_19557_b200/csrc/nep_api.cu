@@ -512,9 +512,9 @@ static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64
         c->cap_Sb = Sb;
     }
     if (!b.lacc) {   // loss accumulators and the block ticket: zero once, the loss kernel re-arms them itself
-        ALLOC(c, b.lacc, double, 8); ALLOC(c, b.counter, unsigned, 4);
+        ALLOC(c, b.lacc, double, 8); ALLOC(c, b.counter, unsigned, 64);
         NEP_CUDA(c, cudaMemsetAsync(b.lacc, 0, 64, c->stream));
-        NEP_CUDA(c, cudaMemsetAsync(b.counter, 0, 16, c->stream));
+        NEP_CUDA(c, cudaMemsetAsync(b.counter, 0, 256, c->stream));
     }
     // per-batch tables: one pinned host block, one device block, one copy per nep_set_batch
     const size_t need = 16 * (size_t)nbs + 8 * (size_t)Sb + 4 * (size_t)Sb * (2 + m.T) + 64;

@@ -97,7 +97,7 @@ struct BatchDev {
     float* eps;    // [Sb]       dL/dE_s
     float* G;      // [Sb][9]    dL/dW_s
     double* lacc;  // [8] sums: (dE)^2, |dF|^2, (dW)^2, spare ; loss4 at [4..7]
-    unsigned* counter;   // [4] block ticket of the loss kernel
+    unsigned* counter;   // [64] [0]: block ticket of the loss kernel; [8 + 4 k ..]: work queue of persistent sweep k (next, done)
 };
 
 struct Profiler {

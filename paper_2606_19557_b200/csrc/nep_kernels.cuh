@@ -22,7 +22,7 @@ struct StepArgs {
     int nchunks;   // angular channel chunks (blockIdx.y)
 };
 
-constexpr int PAIR_TB = 64;   // threads per block of the pair sweeps (2 slices)
+constexpr int PAIR_TB = 128;   // threads per block of the pair sweeps (2 slices)
 
 struct Lane {
     int w, lane, ds, sb, bbase, ti;
@@ -38,6 +38,44 @@ __device__ __forceinline__ int tile_type_of(const BatchDev& b, int tile, int T)
 #pragma unroll 1
     while (t + 1 < T && tile >= b.tile_start[t + 1]) ++t;
     return t;
+}
+
+// lane state for batch slice w (w < a.b.nbs)
+__device__ __forceinline__ void lane_init_slice(const StepArgs& a, Lane& L, int w)
+{
+    L.w = w;
+    L.lane = threadIdx.x & 31;
+    const int4 bi = __ldg(a.b.binfo + w);
+    L.ds = bi.x; L.sb = bi.y; L.bbase = bi.z;
+    L.ib = (unsigned)w * WARP + L.lane;
+    L.ti = __ldg(a.d.type_p + (size_t)L.ds * WARP + L.lane);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Persistent sweeps: a resident wave of warps takes work units (slices, or slice x pass) from a queue in global memory
+// (queue[0] = next unit, queue[1] = blocks that have finished; the last block to finish re-arms both: kernels of one stream
+// do not overlap).  The unit after the current one is fetched early, and the per-atom rows it will load in its prologue are
+// requested into L2 (cp.async.bulk.prefetch.L2, one instruction per contiguous block of rows) while the pairs of the current
+// unit are processed: the prologue then waits for L2 hits instead of DRAM.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned wq_issue(unsigned* queue)   // lane 0 takes a ticket; the value is valid after wq_value
+{
+    unsigned u = 0u;
+    if ((threadIdx.x & 31) == 0) u = atomicAdd(queue, 1u);
+    return u;
+}
+__device__ __forceinline__ unsigned wq_value(unsigned ticket) { return __shfl_sync(0xffffffffu, ticket, 0); }
+__device__ __forceinline__ void wq_finish(unsigned* queue)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(queue + 1, 1u) == gridDim.x * gridDim.y * gridDim.z - 1u) { queue[0] = 0u; queue[1] = 0u; __threadfence(); }
+    }
+}
+__device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes)   // bytes: a multiple of 16
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(p), "r"(bytes) : "memory");
 }
 
 // false if the warp is beyond the batch (whole warp returns together)
@@ -129,13 +167,32 @@ __device__ __forceinline__ void sweep_pairs(const float4* __restrict__ rec, int 
 {
     sweep_pairs(rec, width, cnt, stage, [](bool, const float4&) {}, body);
 }
+// the same pipeline for a block of TB threads (staging cells of successive stages are TB apart)
+template <int TB, class Body>
+__device__ __forceinline__ void sweep_pairs_tb(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body&& body)
+{
+#pragma unroll
+    for (int st = 0; st < SWEEP_STAGES; ++st) {
+        if (st < width) cp_async16(stage + st * TB, rec + (size_t)st * WARP);
+        cp_async_commit();
+    }
+    for (int s = 0; s < width; ++s) {
+        cp_async_wait<SWEEP_STAGES - 1>();
+        float4* cell = stage + (s % SWEEP_STAGES) * TB;
+        const float4 cur = *cell;
+        if (s + SWEEP_STAGES < width) cp_async16(cell, rec + (size_t)(s + SWEEP_STAGES) * WARP);
+        cp_async_commit();
+        if (s < cnt) body(cur);
+    }
+    cp_async_wait<0>();
+}
 
 // Two slots per iteration: body2(record of slot s, record of slot s + 1, has_second) for s = 0, 2, 4, ... < cnt.
 // The dependent chains of a pair (distance, cutoff polynomial, Chebyshev recurrence) are long and a sweep runs two
 // warps per scheduler, so the arithmetic of two pairs is interleaved to fill the pipe.  When the lane has no second
 // record the first one is passed again with has_second = false (finite values that the body multiplies by zero).
 // stage: 4 staging cells per thread, SWEEP2_TB apart.
-constexpr int SWEEP2_TB = 64;
+constexpr int SWEEP2_TB = 128;
 constexpr int SWEEP2_SMEM_BYTES = SWEEP2_TB * 16 * 4;
 template <int TB, class Body2>
 __device__ __forceinline__ void sweep_pairs2(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body2&& body2)

@@ -18,30 +18,32 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
     const int nthreads = gridDim.x * blockDim.x;
     for (int i = gid; i < a.m.npar; i += nthreads) a.g[i] = 0.0f;
     double sF = 0.0, sE = 0.0, sW = 0.0, sB = 0.0;
-    if (gid < a.b.NBP) {
-        const int w = gid >> 5, lane = gid & 31;
+    // grid-stride: at most two blocks per SM, so that the same-address atomics below number a few hundred, not one set per 256 atoms
+    for (int64_t ia = gid; ia < a.b.NBP; ia += nthreads) {
+        const int w = (int)(ia >> 5), lane = (int)(ia & 31);
         const int4 bi = __ldg(a.b.binfo + w);
         const bool valid = __ldg(a.d.type_p + (size_t)bi.x * WARP + lane) >= 0;
         const float c = (float)(2.0 * dlamF / (3.0 * a.b.nrmN));
         const float* Fp = sb_ptr(a.b.F, w, 3, lane);
         const float* Fl = sb_ptr(a.d.Flab, bi.x, 3, lane);
         float* up = sb_ptr(a.b.u, w, 3, lane);
+        float s2 = 0.0f;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             const float dF = valid ? Fp[k * WARP] - __ldg(Fl + k * WARP) : 0.0f;
-            sF += (double)dF * (double)dF;
+            s2 = fmaf(dF, dF, s2);
             up[k * WARP] = c * dF;
         }
+        sF += (double)s2;
     }
-    if (gid < a.b.Sb) {
-        const int sb = gid;
+    for (int sb = gid; sb < a.b.Sb; sb += nthreads) {
         const int sid = a.b.bsid[sb];
         const double n = (double)a.b.bnat[sb];
         const double dE = a.b.Es[sb] - a.d.Elab[sid];
-        sE = (dE / n) * (dE / n);                                                   // Eq. 5
+        sE += (dE / n) * (dE / n);                                                  // Eq. 5
         const float eps = (float)(2.0 * dlamE * dE / (a.b.nrmS * n * n));
         a.b.eps[sb] = eps;
-        sB = (double)eps * n;
+        sB += (double)eps * n;
         const bool hv = a.d.hasv[sid] != 0;
 #pragma unroll
         for (int k = 0; k < 9; ++k) {
@@ -80,8 +82,9 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
 
 int launch_loss(nep_ctx* c, const StepArgs& a)
 {
-    const int64_t n = std::max<int64_t>(c->b.NBP, 1);
-    NEP_LAUNCH(c, "k_loss", k_loss, (unsigned)((n + 255) / 256), 256, 0, a, (float)c->lamE, (float)c->lamF, (float)c->lamV,
+    const int64_t n = std::max<int64_t>(std::max<int64_t>(c->b.NBP, c->b.Sb), 1);
+    const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 2 * (int64_t)c->sm_count);
+    NEP_LAUNCH(c, "k_loss", k_loss, grid, 256, 0, a, (float)c->lamE, (float)c->lamF, (float)c->lamV,
                c->lamE, c->lamF, c->lamV);
     return NEP_OK;
 }
