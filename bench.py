@@ -162,7 +162,12 @@ def dp_exchange(nep):
         allreduce_grad_loss(*DP["views"])
 
 
-def one_step(nep, lam):
+def one_step(nep, lam, graph=False):
+    """One training step.  graph: nep_train_step, the step's kernels replayed as one CUDA graph launch (single GPU only: the
+    data-parallel step has the all-reduce between nep_loss_grad and nep_adam_step)."""
+    if graph and DP["views"] is None:
+        nep.train_step(lam[0], lam[1], lam[2], LR, use_graph=True)
+        return
     nep.forward_device()
     nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
     dp_exchange(nep)
@@ -174,12 +179,13 @@ def e2e_step(nep, lam, ids):
     (nep_set_batch copies them and the slice tables to the device), the loss comes back (nep_loss_grad -> host)."""
     nep.set_batch(ids)
     dp_whole_batch(nep)
+    if DP["views"] is None:
+        nep.train_step(lam[0], lam[1], lam[2], LR, use_graph=True)   # one graph launch (captured again when the batch's shape changes)
+        return nep.get_loss()                      # the step's loss terms -> host
     nep.forward_device()
     nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
     dp_exchange(nep)
     nep.adam_step(LR)                              # queued before the read-back below synchronises
-    if DP["views"] is None:
-        return nep.get_loss()                      # the step's loss terms -> host
     return DP["views"][1].cpu().numpy()            # the whole batch's loss terms -> host
 
 
@@ -231,7 +237,7 @@ def run_ours(args):
         nep.set_batch(None)
         dp_whole_batch(nep)
     for i in range(max(args.warmup, 3)):
-        set_b(i); one_step(nep, lam)
+        set_b(i); one_step(nep, lam, graph=i % 2 == 1)
     torch.cuda.synchronize()
 
     # ---- timed region: K steps, CUDA events per step on the launching stream, L2 flushed between steps ----
@@ -257,7 +263,7 @@ def run_ours(args):
         nep.profile_pause(not sampled)
         n_prof += int(sampled)
         ev[i][0].record()
-        one_step(nep, lam)
+        one_step(nep, lam, graph=not sampled)      # sampled steps: the three calls, with CUDA events between their kernels
         ev[i][1].record()
     torch.cuda.synchronize()
     t1 = time.time()
@@ -283,9 +289,14 @@ def run_ours(args):
     torch.cuda.synchronize()
     a.record()
     for i in range(K):
-        set_b(i); one_step(nep, lam)
+        set_b(i); one_step(nep, lam, graph=True)
     b.record(); torch.cuda.synchronize()
     ms_b2b = a.elapsed_time(b) / K
+    a.record()
+    for i in range(K):
+        set_b(i); one_step(nep, lam, graph=False)
+    b.record(); torch.cuda.synchronize()
+    ms_b2b_stream = a.elapsed_time(b) / K
 
     # ---- e2e: host ids in, host loss out, every step ----
     e2e_batches = full_batches if not single else [np.arange(w.structures.n_struct, dtype=np.int32)]
@@ -364,11 +375,12 @@ def run_ours(args):
         "config": {"workload": workload_name(w, args), "structures_per_s": structs / (total_ms * 1e-3),
                    "atoms_per_step": atoms // K // world, "pairs_R_per_step": sizes["P_R_b"], "pairs_A_per_step": sizes["P_A_b"],
                    "l2": ("flushed between timed steps (256 MB write)" if flush is not None else "not flushed; per-step working set exceeds L2"),
-                   "ms_per_step_back_to_back_no_flush": ms_b2b, "kernel_events": f"every {PROF_EVERY}th timed step ({n_prof} of {K})", "setup_s": setup,
+                   "ms_per_step_back_to_back_no_flush": ms_b2b, "ms_per_step_back_to_back_three_calls": ms_b2b_stream,
+                   "step_call": "nep_train_step (one CUDA graph launch per step; every 5th timed step runs nep_forward + nep_loss_grad + nep_adam_step with per-kernel CUDA events)", "kernel_events": f"every {PROF_EVERY}th timed step ({n_prof} of {K})", "setup_s": setup,
                    "device_bytes": nep.bytes_allocated, "parallelism": (f"dp{world}: structures sharded, whole batch = {world} x {w.batch_size} structures, one NCCL all-reduce of g "
                                     f"[{w.model.n_par} fp32] + 4 loss terms per step" if use_dist else "dp1 (one GPU, no collective)")},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
-                "what": "per step: nep_set_batch(host ids) + nep_forward + nep_loss_grad + nep_adam_step + nep_get_loss(-> host); geometry cache resident (P:143)"},
+                "what": "per step: nep_set_batch(host ids) + nep_train_step (one graph launch) + nep_get_loss(-> host); geometry cache resident (P:143)"},
         "gpu_launches": int(launches),
         "clocks": clk,
         "roofline": roof,

@@ -166,6 +166,15 @@ int nep_grad_device_ptr(nep_ctx* ctx, float** g, double** loss4);
  * Increments the step count t.  Invalidates the forward results. */
 int nep_adam_step(nep_ctx* ctx, double lr, double beta1, double beta2, double eps, int variant);
 
+/* One training step = nep_forward + nep_loss_grad + nep_adam_step on the current batch, without outputs (the loss terms stay
+ * on the device: nep_get_loss).  use_graph != 0: the step's kernels are captured once into a CUDA graph and replayed with one
+ * launch; loss weights, learning rate and the bias corrections of Eq. 11 are written into the graph's nodes before each
+ * replay, so they may change from step to step.  nep_set_batch, nep_set_batch_normalisers, nep_set_labels and
+ * nep_load_structures invalidate the graph (nep_set_batch only if the batch's shape changes); the first step after that runs as
+ * the three calls, the graph is captured when the same batch is stepped a second time.  Same results as the three calls. */
+int nep_train_step(nep_ctx* ctx, double lambda_E, double lambda_F, double lambda_V, double lr, double beta1, double beta2,
+                   double eps, int variant, int use_graph);
+
 /* Blocks until the context's stream is idle. */
 int nep_synchronize(nep_ctx* ctx);
 

@@ -55,6 +55,7 @@ SIGNATURES = {
     "nep_set_batch_normalisers": (C.c_int, [_P, C.c_int64, C.c_int64, C.c_int64]),
     "nep_grad_device_ptr": (C.c_int, [_P, C.POINTER(_P), C.POINTER(_P)]),
     "nep_adam_step": (C.c_int, [_P, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int]),
+    "nep_train_step": (C.c_int, [_P, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int]),
     "nep_synchronize": (C.c_int, [_P]),
     "nep_launch_count": (C.c_int, [_P, C.POINTER(C.c_int64)]),
     "nep_profile_enable": (C.c_int, [_P, C.c_int]),
@@ -337,6 +338,11 @@ class Nep:
 
     def adam_step(self, lr: float, beta1: float = 0.9, beta2: float = 0.999, eps: float = 1e-8, variant: int = 0):
         self._ck(self._L.nep_adam_step(self._h, lr, beta1, beta2, eps, variant))
+
+    def train_step(self, lambda_E: float, lambda_F: float, lambda_V: float, lr: float, beta1: float = 0.9, beta2: float = 0.999,
+                   eps: float = 1e-8, variant: int = 0, use_graph: bool = True):
+        """forward + loss_grad + adam_step on the current batch as one call (one CUDA graph launch with use_graph)."""
+        self._ck(self._L.nep_train_step(self._h, lambda_E, lambda_F, lambda_V, lr, beta1, beta2, eps, variant, int(use_graph)))
 
     def synchronize(self):
         self._ck(self._L.nep_synchronize(self._h))

@@ -31,18 +31,28 @@ __global__ void __launch_bounds__(256) k_adam(int n, float* __restrict__ theta, 
     }
 }
 
+void adam_args(nep_ctx* c, double lr, double b1, double b2, double eps, int variant, int64_t t, AdamArgs* o)
+{
+    const double bc1 = 1.0 - pow(b1, (double)t), bc2 = 1.0 - pow(b2, (double)t);
+    o->n = c->m.npar; o->theta = c->theta; o->g = c->g; o->m = c->am; o->v = c->av; o->vmax = c->avmax;
+    o->lr = (float)lr; o->beta1 = (float)b1; o->beta2 = (float)b2; o->omb1 = (float)(1.0 - b1); o->omb2 = (float)(1.0 - b2);
+    o->eps = (float)eps; o->inv_bc1 = (float)(1.0 / bc1); o->inv_bc2 = (float)(1.0 / bc2);
+    o->func = variant == 0 ? (const void*)k_adam<0> : (const void*)k_adam<1>;
+    o->ptrs[0] = &o->n; o->ptrs[1] = &o->theta; o->ptrs[2] = &o->g; o->ptrs[3] = &o->m; o->ptrs[4] = &o->v; o->ptrs[5] = &o->vmax;
+    o->ptrs[6] = &o->lr; o->ptrs[7] = &o->beta1; o->ptrs[8] = &o->beta2; o->ptrs[9] = &o->omb1; o->ptrs[10] = &o->omb2;
+    o->ptrs[11] = &o->eps; o->ptrs[12] = &o->inv_bc1; o->ptrs[13] = &o->inv_bc2;
+}
+
 int launch_adam(nep_ctx* c, double lr, double b1, double b2, double eps, int variant)
 {
     c->t_adam += 1;
-    const double bc1 = 1.0 - pow(b1, (double)c->t_adam), bc2 = 1.0 - pow(b2, (double)c->t_adam);
-    const int n = c->m.npar;
-    const unsigned grid = (unsigned)((n + 255) / 256);
-    if (variant == 0)
-        NEP_LAUNCH(c, "k_adam", k_adam<0>, grid, 256, 0, n, c->theta, c->g, c->am, c->av, c->avmax, (float)lr, (float)b1, (float)b2,
-                   (float)(1.0 - b1), (float)(1.0 - b2), (float)eps, (float)(1.0 / bc1), (float)(1.0 / bc2));
-    else
-        NEP_LAUNCH(c, "k_adam", k_adam<1>, grid, 256, 0, n, c->theta, c->g, c->am, c->av, c->avmax, (float)lr, (float)b1, (float)b2,
-                   (float)(1.0 - b1), (float)(1.0 - b2), (float)eps, (float)(1.0 / bc1), (float)(1.0 / bc2));
+    AdamArgs A;
+    adam_args(c, lr, b1, b2, eps, variant, c->t_adam, &A);
+    const unsigned grid = (unsigned)((A.n + 255) / 256);
+    prof_begin(c, "k_adam");
+    cudaError_t e = cudaLaunchKernel(A.func, dim3(grid), dim3(256), A.ptrs, 0, c->stream);
+    prof_end(c);
+    NEP_CUDA(c, e);
     return NEP_OK;
 }
 

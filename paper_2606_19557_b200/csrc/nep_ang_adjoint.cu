@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
     const int nwarp = blockDim.x >> 5;
     const int T = m.T, rows = T * NK;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
-    float* tab_all = smem + SWEEP_SMEM_BYTES / 4;                                   // MULTI: [nwarp][rows][ADJ_TST]; else [nwarp][NK]
+    float* tab_all = smem + PAIR_TB * 16;                                           // MULTI: [nwarp][rows][ADJ_TST]; else [nwarp][NK]
     int* cend_all = reinterpret_cast<int*>(tab_all + (size_t)nwarp * rows * ADJ_TST);   // MULTI: [nwarp][T] end column of each centre type
     const int n0 = blockIdx.y * NCH;
     const int wib = threadIdx.x >> 5;
@@ -103,12 +103,18 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                     pack24(X[n], X2[n]);
                 }
             }
-            sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
-                const PairGeo p = pair_geo(rc4);
-                next_type(p.tj);
+            struct Prep { PairGeo p; float fv[2 * KH]; };
+            auto prep = [&](const float4& rc4, float on) {
+                Prep P;
+                P.p = pair_geo(rc4);
+                P.fv[2 * KH - 1] = 0.0f;
+                cheb_basis<K, false>(P.p.r, rcinv, [&](int k, float fk, float) { P.fv[k] = fk * on; });
+                return P;
+            };
+            auto contract = [&](const Prep& P) {
                 float b[NL], al[NCH];
                 float2 b2[NL / 2];
-                harm24(harm_z(p.z), harm_xy(p.x, p.y), b);
+                harm24(harm_z(P.p.z), harm_xy(P.p.x, P.p.y), b);
                 pack24(b, b2);
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) {
@@ -117,15 +123,17 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                     for (int l = 0; l < NL / 2; ++l) s1 = __ffma2_rn(X2[n][l], b2[l], s1);
                     al[n] = s1.x + s1.y;
                 }
-                float fv[2 * KH];
-                fv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, false>(p.r, rcinv, [&](int k, float fk, float) { fv[k] = fk; });
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) {
                     const float2 aa = dup2(al[n]);
 #pragma unroll
-                    for (int k = 0; k < KH; ++k) acc2[n][k] = __ffma2_rn(aa, make_float2(fv[2 * k], fv[2 * k + 1]), acc2[n][k]);
+                    for (int k = 0; k < KH; ++k) acc2[n][k] = __ffma2_rn(aa, make_float2(P.fv[2 * k], P.fv[2 * k + 1]), acc2[n][k]);
                 }
+            };
+            sweep_pairs2<PAIR_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+                const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
+                contract(A);
+                contract(B);
             });
         }
         if (!MULTI || blockIdx.z == 1) {
@@ -143,34 +151,43 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             const float uix = ui[0], uiy = ui[WARP], uiz = ui[2 * WARP];
             const float* ub = a.b.u;
             const int bbase = L.bbase;
-            sweep_pairs(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
-                const PairGeo p = pair_geo(rc4);
-                next_type(p.tj);
-                const Tangent Tg = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
+            struct Prep { PairGeo p; Tangent T; float fv[2 * KH], dfv[2 * KH]; };
+            auto prep = [&](const float4& rc4, float on) {
+                Prep P;
+                P.p = pair_geo(rc4);
+                P.T = pair_tangent(ub, bbase, P.p, uix, uiy, uiz, G);
+                P.fv[2 * KH - 1] = 0.0f; P.dfv[2 * KH - 1] = 0.0f;
+                cheb_basis<K, true>(P.p.r, rcinv, [&](int k, float fk, float dfk) { P.fv[k] = fk * on; P.dfv[k] = dfk * on; });
+                return P;
+            };
+            auto contract = [&](const Prep& P) {
                 float b[NL], bd[NL], be[NCH], de[NCH];
                 float2 b2[NL / 2], bd2[NL / 2];
-                const HarmZ hz = harm_z(p.z);
-                const HarmXY hxy = harm_xy(p.x, p.y);
+                const HarmZ hz = harm_z(P.p.z);
+                const HarmXY hxy = harm_xy(P.p.x, P.p.y);
                 harm24(hz, hxy, b);
-                harm24_tangent(hz, hxy, Tg.rx, Tg.ry, Tg.rz, bd);
+                harm24_tangent(hz, hxy, P.T.rx, P.T.ry, P.T.rz, bd);
                 pack24(b, b2); pack24(bd, bd2);
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) {
                     float2 s1 = make_float2(0.0f, 0.0f), s2 = make_float2(0.0f, 0.0f);
 #pragma unroll
                     for (int l = 0; l < NL / 2; ++l) { s1 = __ffma2_rn(X2[n][l], b2[l], s1); s2 = __ffma2_rn(X2[n][l], bd2[l], s2); }
-                    be[n] = (s1.x + s1.y) * Tg.t; de[n] = s2.x + s2.y;
+                    be[n] = (s1.x + s1.y) * P.T.t; de[n] = s2.x + s2.y;
                 }
-                float fv[2 * KH], dfv[2 * KH];
-                fv[2 * KH - 1] = 0.0f; dfv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, true>(p.r, rcinv, [&](int k, float fk, float dfk) { fv[k] = fk; dfv[k] = dfk; });
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) {
                     const float2 dd = dup2(de[n]), bb = dup2(be[n]);
 #pragma unroll
                     for (int k = 0; k < KH; ++k)
-                        acc2[n][k] = __ffma2_rn(dd, make_float2(fv[2 * k], fv[2 * k + 1]), __ffma2_rn(bb, make_float2(dfv[2 * k], dfv[2 * k + 1]), acc2[n][k]));
+                        acc2[n][k] = __ffma2_rn(dd, make_float2(P.fv[2 * k], P.fv[2 * k + 1]),
+                                                __ffma2_rn(bb, make_float2(P.dfv[2 * k], P.dfv[2 * k + 1]), acc2[n][k]));
                 }
+            };
+            sweep_pairs2<PAIR_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+                const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
+                contract(A);
+                contract(B);
             });
         }
         if (MULTI) {
@@ -390,7 +407,7 @@ int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
         constexpr int NK = NCH * K;
         if (m.T == 1) {
             const int nw = PAIR_TB / WARP;
-            const size_t smem = (size_t)SWEEP_SMEM_BYTES + 4 * (size_t)nw * NK;
+            const size_t smem = (size_t)PAIR_TB * 64 + 4 * (size_t)nw * NK;
             NEP_LAUNCH(c, "k_ang_adjoint", (k_ang_adjoint<NCH, K, false>), dim3((unsigned)((c->b.nbs + nw - 1) / nw), a.nchunks), nw * WARP, smem, a);
         } else {
             constexpr int NKP = (NK + 3) & ~3;

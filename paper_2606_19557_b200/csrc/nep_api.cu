@@ -178,6 +178,8 @@ int nep_destroy(nep_ctx* c)
 {
     if (!c) return NEP_OK;
     cudaStreamSynchronize(c->stream);
+    graph_drop(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     std::vector<void*> a = c->allocs;
     for (void* p : a) dev_free(c, p);
     if (c->h_stage) cudaFreeHost(c->h_stage);
@@ -198,6 +200,7 @@ static void free_dataset(nep_ctx* c)
     for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
     memset(&d, 0, sizeof d);
     c->have_data = c->have_labels = c->have_nbrs = c->forward_valid = c->grad_valid = c->loss_valid = false;
+    ++c->graph_gen;
 }
 
 static int upload_labels(nep_ctx* c, const double* E, const double* F, const double* W, const unsigned char* hv)
@@ -230,6 +233,7 @@ static int upload_labels(nep_ctx* c, const double* E, const double* F, const dou
     dev_free(c, (void*)d.Elab); dev_free(c, (void*)d.Flab); dev_free(c, (void*)d.Wlab); dev_free(c, (void*)d.hasv);
     d.Elab = dE; d.Flab = dF; d.Wlab = dW; d.hasv = dh;
     c->h_Flab.swap(hF); c->h_hasv.swap(hasv);
+    ++c->graph_gen;
     c->have_labels = true;
     c->grad_valid = false;
     return NEP_OK;
@@ -314,6 +318,7 @@ int nep_set_labels(nep_ctx* c, const double* E, const double* F, const double* W
         for (int sid : c->h_bsid) sv += c->h_hasv[sid];
         c->b.Sv = sv;
         c->b.nrmS = (double)c->b.Sb; c->b.nrmN = (double)c->b.Nb; c->b.nrmV = (double)sv;
+        ++c->graph_gen;
     }
     return rc;
 }
@@ -562,10 +567,12 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
     for (int t = 0; t < T; ++t) { b.tile_start[t] = ntiles; ntiles += (int)((tot[t] + TM - 1) / TM); }
     for (int t = T; t <= MAX_T; ++t) b.tile_start[t] = ntiles;
     c->forward_valid = c->grad_valid = false;
+    const BatchDev b_before = c->b;            // a batch of the same shape in the same buffers leaves a captured step graph valid
     int rc = ensure_batch_capacity(c, std::max<int64_t>(nbs64 * WARP, WARP), std::max(Sb, 1), std::max(nbs, 1), std::max<int64_t>((int64_t)ntiles * TM, TM));
     if (rc) {   // no batch is selected after a failed allocation: the step calls launch nothing
         b.Sb = b.Sv = 0; b.Nb = 0; b.nbs = 0; b.NBP = 0; b.ntiles = 0;
         c->h_bsid.clear(); c->h_bfoff.clear();
+        ++c->graph_gen;
         return rc;
     }
     // tables, packed: binfo [nbs] int4 | bfoff [Sb] int64 | bsid [Sb] | bnat [Sb] | bsoff [Sb][T]
@@ -601,6 +608,7 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
     if (bytes) NEP_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, bytes, cudaMemcpyHostToDevice, c->stream));
     c->h_bsid.assign(bsid, bsid + Sb); c->h_bfoff.assign(bfoff, bfoff + Sb); c->PRb = PRb; c->PAb = PAb;
     c->forward_valid = c->grad_valid = false;
+    if (memcmp(&b_before, &c->b, sizeof(BatchDev)) != 0) ++c->graph_gen;
     return launch_build_alist(c);
 }
 
@@ -663,6 +671,7 @@ int nep_set_batch_normalisers(nep_ctx* c, int64_t n_struct, int64_t n_atoms, int
         return fail(c, NEP_EINVAL, "the whole batch cannot be smaller than this context's share of it");
     c->b.nrmS = (double)n_struct; c->b.nrmN = (double)n_atoms; c->b.nrmV = (double)n_virial;
     c->grad_valid = false;
+    ++c->graph_gen;
     return NEP_OK;
 }
 

@@ -151,6 +151,13 @@ struct nep_ctx {
 
     int64_t launches = 0;
     nep::Profiler prof;
+
+    // one training step as a CUDA graph (nep_graph.cu); graph_gen is bumped by every call that changes pointers or launch shapes
+    cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr; cudaStream_t cap_stream = nullptr;
+    cudaGraphNode_t graph_loss_node = nullptr, graph_adam_node = nullptr;
+    unsigned graph_loss_grid = 0, graph_adam_grid = 0;
+    int64_t graph_gen = 0, graph_built_gen = -1, graph_seen_gen = -1;
+    int graph_variant = 0, graph_launches = 0;
 };
 
 namespace nep {
@@ -180,6 +187,7 @@ int launch_scaler_from_range(nep_ctx* c, const float* d_rng, float* d_s);   //  
 int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW);  // nep_misc.cu: slice-blocked -> batch order
 int launch_gather_q(nep_ctx* c, float* dq);                    // [N_b][D]
 int launch_build_alist(nep_ctx* c);                            // nep_misc.cu     : type-sorted atom list of the batch
+void graph_drop(nep_ctx* c);                                   // nep_graph.cu    : releases the captured step graph
 int ann_tile_m(const nep_ctx* c);                              // nep_ann.cu      : atoms per network tile for this model
 
 }  // namespace nep

@@ -376,6 +376,19 @@ __device__ __forceinline__ Tangent pair_tangent(const float* __restrict__ ub, in
         NEP_CUDA((c), cudaGetLastError());                                         \
     } while (0)
 
+// kernel + argument blocks of the two step kernels whose scalar arguments change from step to step (loss weights, learning
+// rate, Adam bias corrections): used for the direct launch and to re-parameterise their nodes in a captured step graph
+struct LossArgs {
+    StepArgs a; float lamE, lamF, lamV; double dlamE, dlamF, dlamV;
+    const void* func; void* ptrs[7];
+};
+struct AdamArgs {
+    int n; float *theta; const float* g; float *m, *v, *vmax; float lr, beta1, beta2, omb1, omb2, eps, inv_bc1, inv_bc2;
+    const void* func; void* ptrs[14];
+};
+void loss_args(nep_ctx* c, const StepArgs& a, LossArgs* o);
+void adam_args(nep_ctx* c, double lr, double b1, double b2, double eps, int variant, int64_t t, AdamArgs* o);
+
 // channels per thread for the angular sweeps: 3, 4 or 5 (fewer channels run as 3 with zero coefficients)
 inline int pick_nch(int nA)
 {

@@ -80,12 +80,26 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
     }
 }
 
+void loss_args(nep_ctx* c, const StepArgs& a, LossArgs* o)
+{
+    o->a = a;
+    o->lamE = (float)c->lamE; o->lamF = (float)c->lamF; o->lamV = (float)c->lamV;
+    o->dlamE = c->lamE; o->dlamF = c->lamF; o->dlamV = c->lamV;
+    o->func = (const void*)k_loss;
+    o->ptrs[0] = &o->a; o->ptrs[1] = &o->lamE; o->ptrs[2] = &o->lamF; o->ptrs[3] = &o->lamV;
+    o->ptrs[4] = &o->dlamE; o->ptrs[5] = &o->dlamF; o->ptrs[6] = &o->dlamV;
+}
+
 int launch_loss(nep_ctx* c, const StepArgs& a)
 {
     const int64_t n = std::max<int64_t>(std::max<int64_t>(c->b.NBP, c->b.Sb), 1);
     const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 2 * (int64_t)c->sm_count);
-    NEP_LAUNCH(c, "k_loss", k_loss, grid, 256, 0, a, (float)c->lamE, (float)c->lamF, (float)c->lamV,
-               c->lamE, c->lamF, c->lamV);
+    LossArgs A;
+    loss_args(c, a, &A);
+    prof_begin(c, "k_loss");
+    cudaError_t e = cudaLaunchKernel(A.func, dim3(grid), dim3(256), A.ptrs, 0, c->stream);
+    prof_end(c);
+    NEP_CUDA(c, e);
     return NEP_OK;
 }
 

@@ -315,3 +315,37 @@ def test_full_training_steps_track_the_oracle():
     assert np.allclose(Lg, Lo, rtol=1e-3), (Lg, Lo)
     assert Lo[-1] < Lo[0]
     assert H.relnorm(thg, th) < 1e-4
+
+
+@pytest.mark.parametrize("name", ["cfg1a", "cfg3"])
+def test_train_step_graph_matches_the_three_calls(name):
+    """nep_train_step (one CUDA graph launch per step, loss weights / learning rate / bias corrections re-written into its nodes)
+    against nep_forward + nep_loss_grad + nep_adam_step: same parameters and loss terms, across a change of the loss weights
+    and of the learning rate, a new batch (graph captured again) and both Adam variants; the first step also against the oracle."""
+    prob = _prob(name)
+    S = prob.workload.structures.n_struct
+    sched = [((1.0, 1.0, 1.0), 1e-3, 0), ((1.0, 1.0, 1.0), 1e-3, 0), ((2.0, 0.5, 3.0), 5e-4, 0), ((2.0, 0.5, 3.0), 2e-4, 0)]
+    with H.make_gpu(prob) as ref, H.make_gpu(prob) as gr, H.make_gpu(prob) as st:
+        def run(batch, sched, check_oracle=False):
+            for nep in (ref, gr, st):
+                nep.set_batch(batch)
+            for i, (lam, lr, variant) in enumerate(sched):
+                ref.forward_device(); ref.loss_grad(*lam, fetch_loss=False); ref.adam_step(lr, variant=variant)
+                gr.train_step(*lam, lr, variant=variant, use_graph=True)
+                st.train_step(*lam, lr, variant=variant, use_graph=False)
+                l_ref, l_gr, l_st = ref.get_loss(), gr.get_loss(), st.get_loss()
+                assert np.allclose(l_gr, l_ref, rtol=1e-5, atol=1e-14) and np.allclose(l_st, l_ref, rtol=1e-5, atol=1e-14)
+                th_ref, th_gr, th_st = ref.get_params(), gr.get_params(), st.get_params()
+                scale = max(1.0, float(np.max(np.abs(th_ref))))
+                assert np.max(np.abs(th_gr - th_ref)) <= 2e-6 * scale and np.max(np.abs(th_st - th_ref)) <= 2e-6 * scale
+                if check_oracle and i == 0:
+                    l4o, go = O.loss_grad(prob.data, prob.theta, prob.scaler, lam, batch=None if batch is None else list(batch))
+                    th = prob.theta.copy(); n = th.size
+                    O.adam_step(th, go, np.zeros(n), np.zeros(n), np.zeros(n), 0, lr)
+                    assert np.allclose(l_gr, l4o, rtol=2e-4) and np.max(np.abs(th_gr - th)) < 1e-5
+        run(None, sched, check_oracle=True)
+        sub = np.arange(S, dtype=np.int32)[::2]
+        run(sub, sched[:2])                                   # new batch: the step is captured again
+        run(sub, [((1.0, 1.0, 1.0), 1e-3, 1)] * 2)            # other Adam variant: other kernel, captured again
+        assert gr.get_adam_state()[3] == ref.get_adam_state()[3] == st.get_adam_state()[3]
+        assert gr.launch_count() == ref.launch_count()        # a replayed graph counts the kernels it launches
