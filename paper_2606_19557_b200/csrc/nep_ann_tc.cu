@@ -38,7 +38,7 @@ constexpr int TC_TM = 128;      // atoms per tile = threads per block = TMEM lan
 struct TcLay {
     int DP8, HP8, HP16, DP16, KMAX, TK, TKRP, nR4, NC16, MA;
     int cR2, cACC, ncols;                         // TMEM columns: R1 at 0
-    int oW1H, oW1L, oW2H, oW2L, ob0, ow1, osc, ocR, oQBT, oQDT, oGT, oET, ogw1, oStg, oBar, total;   // float offsets
+    int oW1H, oW1L, oW2H, oW2L, ob0, ow1, osc, ocR, oQBT, oQDT, oGT, oET, ogw1, oStg, oEi, oBar, total;   // float offsets
     int ldQ, ldG;                                 // rows' of the transposed buffers (odd)
 };
 
@@ -69,6 +69,7 @@ static TcLay tc_layout(const ModelDev& m, bool bwd)
     l.ocR = take(bwd ? l.TK * l.nR4 : m.nR * l.TKRP);
     l.ogw1 = take(l.HP8);
     l.oStg = take(m.per_type);
+    l.oEi = take(bwd ? 0 : 4 * TC_TM);
     l.oBar = take(8);
     l.total = o;
     return l;
@@ -86,11 +87,11 @@ __device__ __forceinline__ void tc_load_weights(const StepArgs& a, const TcLay& 
     const float* th = a.theta + (size_t)t * m.per_type;
     float* stg = sm + l.oStg;
 #pragma unroll 8
-    for (int i = threadIdx.x; i < m.per_type; i += TC_TM) stg[i] = __ldg(th + i);
-    for (int i = threadIdx.x; i < l.DP8; i += TC_TM) sm[l.osc + i] = (i < m.D) ? __ldg(a.scaler + i) : 0.0f;
+    for (int i = threadIdx.x; i < m.per_type; i += blockDim.x) stg[i] = __ldg(th + i);
+    for (int i = threadIdx.x; i < l.DP8; i += blockDim.x) sm[l.osc + i] = (i < m.D) ? __ldg(a.scaler + i) : 0.0f;
     __syncthreads();
 #pragma unroll 4
-    for (int i = threadIdx.x; i < l.DP8 * l.HP16; i += TC_TM) {
+    for (int i = threadIdx.x; i < l.DP8 * l.HP16; i += blockDim.x) {
         const int c = i / (4 * l.HP16), rem = i - c * 4 * l.HP16, mu = rem >> 2, v = 4 * c + (rem & 3);
         const float wv = (mu < m.H && v < m.D) ? stg[mu * m.D + v] * sm[l.osc + v] : 0.0f;
         const float hi = tf32_rn(wv);
@@ -98,14 +99,14 @@ __device__ __forceinline__ void tc_load_weights(const StepArgs& a, const TcLay& 
         if (SPLIT) sm[l.oW1L + i] = tf32_rn(wv - hi);
     }
 #pragma unroll 4
-    for (int i = threadIdx.x; i < l.HP8 * l.DP16; i += TC_TM) {
+    for (int i = threadIdx.x; i < l.HP8 * l.DP16; i += blockDim.x) {
         const int c = i / (4 * l.DP16), rem = i - c * 4 * l.DP16, v = rem >> 2, mu = 4 * c + (rem & 3);
         const float wv = (mu < m.H && v < m.D) ? stg[mu * m.D + v] * sm[l.osc + v] : 0.0f;
         const float hi = tf32_rn(wv);
         sm[l.oW2H + i] = hi;
         if (SPLIT) sm[l.oW2L + i] = tf32_rn(wv - hi);
     }
-    for (int i = threadIdx.x; i < l.HP8; i += TC_TM) {
+    for (int i = threadIdx.x; i < l.HP8; i += blockDim.x) {
         sm[l.ob0 + i] = (i < m.H) ? stg[m.H * m.D + i] : 0.0f;
         sm[l.ow1 + i] = (i < m.H) ? stg[m.H * m.D + m.H + i] : 0.0f;
     }
@@ -141,57 +142,81 @@ __device__ __forceinline__ void tc_gemm_ts(uint32_t d, uint32_t acol, const floa
 }
 
 // ------------------------------------------------------------------------------------------------
+// Thread layout of both kernels: NT threads per atom (NT = 2 or 4), block = 128 NT threads.  Warp w works on the TMEM lanes
+// of quarter w & 3 (the hardware lets a warp touch only lanes 32 (w % 4) ..), i.e. on atom am = 32 (w & 3) + lane of the tile;
+// the NT warps that share a quarter split every per-atom loop by CHUNKS of 8 columns (the unit of a TMEM load / store):
+// thread part h = w >> 2 takes the chunks c with c % NT == h.
+// ------------------------------------------------------------------------------------------------
+struct TcThread {
+    int tid, w, lane, q, h, am;
+    uint32_t tb;         // TMEM address of this thread's lane, column 0 of the block's allocation
+};
+__device__ __forceinline__ TcThread tc_thread(uint32_t tcol0)
+{
+    TcThread t;
+    t.tid = threadIdx.x; t.w = t.tid >> 5; t.lane = t.tid & 31; t.q = t.w & 3; t.h = t.w >> 2; t.am = 32 * t.q + t.lane;
+    t.tb = tcol0 + ((uint32_t)(32 * t.q) << 16);
+    return t;
+}
+
+// ------------------------------------------------------------------------------------------------
 // S3
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(TC_TM) k_ann_fwd_tc(StepArgs a, TcLay l)
+template <int NT>
+__global__ void __launch_bounds__(TC_TM * NT) k_ann_fwd_tc(StepArgs a, TcLay l)
 {
     extern __shared__ __align__(128) float sm[];
     const ModelDev& m = a.m;
     uint64_t* mbar = reinterpret_cast<uint64_t*>(sm + l.oBar);
     uint32_t* tslot = reinterpret_cast<uint32_t*>(mbar + 1);
-    const int tid = threadIdx.x, w = tid >> 5;
-    if (tid == 0) mbar_init(mbar, 1);
-    if (w == 0) tmem_alloc(tslot, l.ncols);
+    if (threadIdx.x == 0) mbar_init(mbar, 1);
+    if (threadIdx.x < 32) tmem_alloc(tslot, l.ncols);
     fence_before();
     __syncthreads();
     fence_after();
     const uint32_t tcol0 = *tslot;
-    const uint32_t tb = tcol0 + ((uint32_t)(32 * w) << 16);      // this thread's lane
+    const TcThread T = tc_thread(tcol0);
+    const int tid = T.tid, h = T.h;
+    const uint32_t tb = T.tb;
     const uint32_t idesc1 = make_idesc_tf32(128, l.HP16), idesc2 = make_idesc_tf32(128, l.DP16);
     const int tbase = a.b.ntiles / (int)gridDim.x, trem = a.b.ntiles - tbase * (int)gridDim.x;
     const int tile0 = (int)blockIdx.x * tbase + min((int)blockIdx.x, trem), tile1 = tile0 + tbase + ((int)blockIdx.x < trem ? 1 : 0);
     uint32_t phase = 0;
     int cur_t = -1;
     const float b1 = a.theta[m.o_b1];
-    #pragma unroll 1
+    float* eis = sm + l.oEi;                       // [NT][128] partial E_i of the thread parts
+#pragma unroll 1
     for (int tile = tile0; tile < tile1; ++tile) {
         const int t = tile_type_of(a.b, tile, m.T);
         if (t != cur_t) {
             cur_t = t;
             __syncthreads();                       // every thread is done with the previous species' tables
             tc_load_weights<true>(a, l, sm, t);
-            #pragma unroll 4
-            for (int i = tid; i < m.nR * l.TKRP; i += TC_TM) {      // cRs[n][T' KRP + k]
+#pragma unroll 4
+            for (int i = tid; i < m.nR * l.TKRP; i += TC_TM * NT) {      // cRs[n][T' KRP + k]
                 const int n = i / l.TKRP, o = i - n * l.TKRP, tj = o / m.KRP, k = o - tj * m.KRP;
                 sm[l.ocR + i] = (k < m.KR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
             }
         }
-        const int ib = a.b.alist[(size_t)tile * TC_TM + tid];
+        const int ib = a.b.alist[(size_t)tile * TC_TM + T.am];
         const float* qp = ib >= 0 ? sb_ptr(a.b.q, ib >> 5, m.D, ib & 31) : nullptr;
-        // ---- A = q (hi | lo) -> TMEM columns [0, DP8) and [KMAX, KMAX + DP8) ----
-        #pragma unroll 1
-        for (int r0 = 0; r0 < l.DP8; r0 += 32) {
-            float qv[32];
-            load_rows<32>(qp, r0, m.D, qv);
+        // ---- A = q (hi | lo) -> TMEM columns [0, DP8) and [KMAX, KMAX + DP8): this thread's chunks, two at a time ----
+#pragma unroll 1
+        for (int c = h; 8 * c < l.DP8; c += 2 * NT) {
+            float qa[8], qb[8];
+            const int cb = c + NT;
+            load_rows<8>(qp, 8 * c, m.D, qa);
+            load_rows<8>(qp, 8 * cb, m.D, qb);      // rows beyond D: zeros
+            float hi[8], lo[8];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                if (r0 + 8 * c < l.DP8) {
-                    float hi[8], lo[8];
+            for (int j = 0; j < 8; ++j) { hi[j] = tf32_rn(qa[j]); lo[j] = tf32_rn(qa[j] - hi[j]); }
+            tmem_st8(tb + 8 * c, hi);
+            tmem_st8(tb + l.KMAX + 8 * c, lo);
+            if (8 * cb < l.DP8) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) { hi[j] = tf32_rn(qv[8 * c + j]); lo[j] = tf32_rn(qv[8 * c + j] - hi[j]); }
-                    tmem_st8(tb + r0 + 8 * c, hi);
-                    tmem_st8(tb + l.KMAX + r0 + 8 * c, lo);
-                }
+                for (int j = 0; j < 8; ++j) { hi[j] = tf32_rn(qb[j]); lo[j] = tf32_rn(qb[j] - hi[j]); }
+                tmem_st8(tb + 8 * cb, hi);
+                tmem_st8(tb + l.KMAX + 8 * cb, lo);
             }
         }
         tmem_st_wait();
@@ -210,24 +235,25 @@ __global__ void __launch_bounds__(TC_TM) k_ann_fwd_tc(StepArgs a, TcLay l)
         fence_after();
         // ---- h = tanh(x - b0), E_i, e -> A of the second product (hi | lo) ----
         float ei = 0.0f;
-        float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TC_TM + tid;
-        #pragma unroll 1
-        for (int c0 = 0; c0 < l.HP8; c0 += 8) {
+        float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TC_TM + T.am;
+#pragma unroll 1
+        for (int c0 = 8 * h; c0 < l.HP8; c0 += 8 * NT) {
             float x[8], hi[8], lo[8];
             tmem_ld8(tb + l.cR2 + c0, x);
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const float w1 = sm[l.ow1 + c0 + j];
-                const float h = tanh_fast(x[j] - sm[l.ob0 + c0 + j]);
-                ei = fmaf(w1, h, ei);
-                const float e = w1 * fmaf(-h, h, 1.0f);
-                hb[(size_t)(c0 + j) * TC_TM] = h;
+                const float hh = tanh_fast(x[j] - sm[l.ob0 + c0 + j]);
+                ei = fmaf(w1, hh, ei);
+                const float e = w1 * fmaf(-hh, hh, 1.0f);
+                hb[(size_t)(c0 + j) * TC_TM] = hh;
                 hi[j] = tf32_rn(e); lo[j] = tf32_rn(e - hi[j]);
             }
             tmem_st8(tb + c0, hi);
             tmem_st8(tb + l.KMAX + c0, lo);
         }
+        eis[h * TC_TM + T.am] = ei;
         tmem_st_wait();
         fence_before();
         __syncthreads();
@@ -239,15 +265,18 @@ __global__ void __launch_bounds__(TC_TM) k_ann_fwd_tc(StepArgs a, TcLay l)
             tc_gemm_ts(d, tcol0, sm + l.oW2L, l.DP16, l.HP8, idesc2, true);
             commit(mbar);
         }
+        if (h == 0 && ib >= 0) {                   // E_i of Eq. 3 (the parts' sums were exchanged before the barrier above)
+            float e = -b1;
+#pragma unroll
+            for (int p = 0; p < NT; ++p) e += eis[p * TC_TM + T.am];
+            a.b.Ei[ib] = e;
+        }
         mbar_wait(mbar, phase); phase ^= 1;
         fence_after();
-        // ---- Fp = dE_i/dq -> global; a_k[T'] from its radial rows ----
-        float fpr[24];
-#pragma unroll
-        for (int j = 0; j < 24; ++j) fpr[j] = 0.0f;
+        // ---- Fp = dE_i/dq -> global (this thread's chunks); a_k[T'] from its radial rows (every part reads them) ----
         float* fpp = ib >= 0 ? sb_ptr(a.b.Fp, ib >> 5, m.D, ib & 31) : nullptr;
-        #pragma unroll 1
-        for (int c0 = 0; c0 < l.DP8; c0 += 8) {
+#pragma unroll 1
+        for (int c0 = 8 * h; c0 < l.DP8; c0 += 8 * NT) {
             float f[8];
             tmem_ld8(tb + l.cR2 + c0, f);
             tmem_ld_wait();
@@ -255,18 +284,21 @@ __global__ void __launch_bounds__(TC_TM) k_ann_fwd_tc(StepArgs a, TcLay l)
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
                     if (c0 + j < m.D) fpp[(size_t)(c0 + j) * WARP] = f[j];
-            if (c0 < 24)
-#pragma unroll
-                for (int cc = 0; cc < 3; ++cc)
-                    if (c0 == 8 * cc)
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) fpr[8 * cc + j] = f[j];
         }
+        float fpr[24];
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+            if (8 * cc < m.nR) tmem_ld8(tb + l.cR2 + 8 * cc, fpr + 8 * cc);
+            else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) fpr[8 * cc + j] = 0.0f;
+            }
+        }
+        tmem_ld_wait();
         if (ib >= 0) {
-            a.b.Ei[ib] = ei - b1;
             float* ar = a.b.arow + (size_t)ib * l.TKRP;
-            #pragma unroll 1
-            for (int o0 = 0; o0 < l.TKRP; o0 += 4) {
+#pragma unroll 1
+            for (int o0 = 4 * h; o0 < l.TKRP; o0 += 4 * NT) {
                 float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
                 for (int n = 0; n < 24; ++n)
@@ -281,7 +313,7 @@ __global__ void __launch_bounds__(TC_TM) k_ann_fwd_tc(StepArgs a, TcLay l)
         fence_before();                            // this tile's TMEM reads are ordered before the next tile's writes
     }
     __syncthreads();
-    if (w == 0) tmem_dealloc(tcol0, l.ncols);
+    if (threadIdx.x < 32) tmem_dealloc(tcol0, l.ncols);
 }
 
 // sum over the 32 lanes of 8 values per lane; lane l returns the total of element 4 b4 + 2 b3 + b2 (bits of l)
@@ -308,20 +340,23 @@ __device__ __forceinline__ float warp_reduce_scatter8(const float* v, int lane)
 // ------------------------------------------------------------------------------------------------
 // S8
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
+template <int NT>
+__global__ void __launch_bounds__(TC_TM * NT) k_ann_bwd_tc(StepArgs a, TcLay l)
 {
     extern __shared__ __align__(128) float sm[];
     const ModelDev& m = a.m;
     uint64_t* mbar = reinterpret_cast<uint64_t*>(sm + l.oBar);
     uint32_t* tslot = reinterpret_cast<uint32_t*>(mbar + 1);
-    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
-    if (tid == 0) mbar_init(mbar, 1);
-    if (w == 0) tmem_alloc(tslot, l.ncols);
+    if (threadIdx.x == 0) mbar_init(mbar, 1);
+    if (threadIdx.x < 32) tmem_alloc(tslot, l.ncols);
     fence_before();
     __syncthreads();
     fence_after();
     const uint32_t tcol0 = *tslot;
-    const uint32_t tb = tcol0 + ((uint32_t)(32 * w) << 16);
+    const TcThread T = tc_thread(tcol0);
+    const int tid = T.tid, h = T.h, lane = T.lane, am = T.am;
+    const uint32_t tb = T.tb;
+    constexpr int NTH = TC_TM * NT;
     const uint32_t idesc1 = make_idesc_tf32(128, l.HP16), idesc2 = make_idesc_tf32(128, l.DP16), idesc3 = make_idesc_tf32(l.MA, l.NC16);
     const int tbase = a.b.ntiles / (int)gridDim.x, trem = a.b.ntiles - tbase * (int)gridDim.x;
     const int tile0 = (int)blockIdx.x * tbase + min((int)blockIdx.x, trem), tile1 = tile0 + tbase + ((int)blockIdx.x < trem ? 1 : 0);
@@ -330,17 +365,18 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
     bool acc_live = false;                        // ACC holds sums of the current species
     float* gw1s = sm + l.ogw1;                    // [HP8] g_w1 of the current species, summed over this block's atoms
     float* QBT = sm + l.oQBT; float* QDT = sm + l.oQDT; float* GT = sm + l.oGT; float* ET = sm + l.oET;
-    const int tq = ((tid >> 2) * l.ldQ) * 4 + (tid & 3), tg = ((tid >> 2) * l.ldG) * 4 + (tid & 3);   // this atom's cell of row 0
+    const int tq = ((am >> 2) * l.ldQ) * 4 + (am & 3), tg = ((am >> 2) * l.ldG) * 4 + (am & 3);   // this atom's cell of row 0
+    const int nrc = (m.nR + 7) >> 3;              // chunks of qd that hold radial rows
 
     // ACC -> g (species t): called by all threads; ends with the tables free for the next species
     auto flush = [&](int t) {
-        // rows of ACC: M = 64: lane < 16 of warp w holds row 16 w + lane; M = 128: row 32 w + lane
-        const int mu = l.MA == 64 ? 16 * w + lane : 32 * w + lane;
+        // rows of ACC: M = 64: lane < 16 of quarter q holds row 16 q + lane; M = 128: row 32 q + lane
+        const int mu = l.MA == 64 ? 16 * T.q + lane : 32 * T.q + lane;
         const bool own = (l.MA == 64 ? lane < 16 : true) && mu < m.H;
         float* gt = a.g + (size_t)t * m.per_type;
         float* stage = QBT;                         // [mu][TK] columns D .. D + TK - 1 of ACC, for the g_cR product below
-        #pragma unroll 1
-        for (int c0 = 0; c0 < l.NC16; c0 += 8) {
+#pragma unroll 1
+        for (int c0 = 8 * h; c0 < l.NC16; c0 += 8 * NT) {
             float v[8];
             tmem_ld8(tb + l.cACC + c0, v);
             tmem_ld_wait();
@@ -355,22 +391,22 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
         }
         fence_before();
         __syncthreads();
-        #pragma unroll 1
-        for (int i = tid; i < m.H; i += TC_TM) atomicAdd(gt + m.H * m.D + m.H + i, gw1s[i]);
+#pragma unroll 1
+        for (int i = tid; i < m.H; i += NTH) atomicAdd(gt + m.H * m.D + m.H + i, gw1s[i]);
         // g_cR[t][T'][n][k] += sum_mu w0s[mu][n] ACC[mu][D + T' KR + k]
-        #pragma unroll 1
-        for (int o = tid; o < m.nR * l.TK; o += TC_TM) {
+#pragma unroll 1
+        for (int o = tid; o < m.nR * l.TK; o += NTH) {
             const int n = o / l.TK, r = o - n * l.TK, tj = r / m.KR, k = r - tj * m.KR;
             const float sn = sm[l.osc + n];
             float s = 0.0f;
-            #pragma unroll 1
+#pragma unroll 4
             for (int mu2 = 0; mu2 < m.H; ++mu2) s = fmaf(sm[l.oStg + mu2 * m.D + n] * sn, stage[mu2 * l.TK + r], s);
             atomicAdd(a.g + m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k, s);
         }
         __syncthreads();
     };
 
-    #pragma unroll 1
+#pragma unroll 1
     for (int tile = tile0; tile < tile1; ++tile) {
         const int t = tile_type_of(a.b, tile, m.T);
         if (t != cur_t) {
@@ -379,16 +415,15 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
             cur_t = t;
             __syncthreads();
             tc_load_weights<false>(a, l, sm, t);
-            #pragma unroll 1
-            for (int i = tid; i < l.HP8; i += TC_TM) gw1s[i] = 0.0f;
-            #pragma unroll 4
-            for (int i = tid; i < l.TK * l.nR4; i += TC_TM) {   // cRt[(T', k)][n]
+            for (int i = tid; i < l.HP8; i += NTH) gw1s[i] = 0.0f;
+#pragma unroll 4
+            for (int i = tid; i < l.TK * l.nR4; i += NTH) {   // cRt[(T', k)][n]
                 const int r = i / l.nR4, n = i - r * l.nR4, tj = r / m.KR, k = r - tj * m.KR;
                 sm[l.ocR + i] = (n < m.nR) ? a.theta[m.o_cR + ((t * m.T + tj) * m.nR + n) * m.KR + k] : 0.0f;
             }
             __syncthreads();                       // cRt is read below before the next barrier
         }
-        const int ib = a.b.alist[(size_t)tile * TC_TM + tid];
+        const int ib = a.b.alist[(size_t)tile * TC_TM + am];
         const bool valid = ib >= 0;
         const float *qp = nullptr, *qdp = nullptr, *Bp = nullptr, *Bdp = nullptr;
         float epsi = 0.0f;
@@ -399,72 +434,61 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
             Bp = sb_ptr(a.d.B, bi.x, l.TK, ln); Bdp = sb_ptr(a.b.Bd, ws, l.TK, ln);
             epsi = a.b.eps[bi.y];
         }
-        // ---- radial tangent qd_n = sum_{T', k} cR[t][T'][n][k] Bd_k[T'];  Bd, B -> transposed operands ----
-        float qdr[24];
+        // ---- B, Bd -> transposed operand columns D .. D + TK - 1: chunks of 8 rows, parts offset by one against the qd chunks ----
+#pragma unroll 1
+        for (int r0 = 8 * ((h + NT - 1) % NT); r0 < l.TK; r0 += 8 * NT) {
+            float bd[8], bv[8];
+            load_rows<8>(Bdp, r0, l.TK, bd);
+            load_rows<8>(Bp, r0, l.TK, bv);
 #pragma unroll
-        for (int n = 0; n < 24; ++n) qdr[n] = 0.0f;
-        #pragma unroll 1
-        for (int r0 = 0; r0 < l.TK; r0 += 16) {
-            float bd[16], bv[16];
-            load_rows<16>(Bdp, r0, l.TK, bd);
-            load_rows<16>(Bp, r0, l.TK, bv);
-#pragma unroll
-            for (int j = 0; j < 16; ++j)
+            for (int j = 0; j < 8; ++j)
                 if (r0 + j < l.TK) {
                     QDT[tq + (m.D + r0 + j) * 4] = tf32_rn(bd[j]);
                     QBT[tq + (m.D + r0 + j) * 4] = tf32_rn(bv[j]);
-                    const float* cr = sm + l.ocR + (r0 + j) * l.nR4;
-#pragma unroll
-                    for (int n4 = 0; n4 < 6; ++n4)
-                        if (4 * n4 < m.nR) {
-                            const float4 c4 = *reinterpret_cast<const float4*>(cr + 4 * n4);
-                            qdr[4 * n4] = fmaf(c4.x, bd[j], qdr[4 * n4]); qdr[4 * n4 + 1] = fmaf(c4.y, bd[j], qdr[4 * n4 + 1]);
-                            qdr[4 * n4 + 2] = fmaf(c4.z, bd[j], qdr[4 * n4 + 2]); qdr[4 * n4 + 3] = fmaf(c4.w, bd[j], qdr[4 * n4 + 3]);
-                        }
                 }
         }
-        // ones column (pairs with gamma: g_b0) and padding columns
-        QBT[tq + (m.D + l.TK) * 4] = valid ? 1.0f : 0.0f;
-        QDT[tq + (m.D + l.TK) * 4] = 0.0f;
-        #pragma unroll 1
-        for (int col = m.D + l.TK + 1; col < l.NC16; ++col) { QBT[tq + col * 4] = 0.0f; QDT[tq + col * 4] = 0.0f; }
-        // ---- q, qd: transposed operands; qd also as A of the first product (TMEM columns [0, DP8)) ----
-        // 16 rows at a time; the radial rows of qd (the first n_R <= 24) are the sums just formed, not loaded
-        auto put16 = [&](int r0, const float* qv, const float* qd) {
+        if (h == NT - 1) {   // ones column (pairs with gamma: g_b0) and padding columns
+            QBT[tq + (m.D + l.TK) * 4] = valid ? 1.0f : 0.0f;
+            QDT[tq + (m.D + l.TK) * 4] = 0.0f;
+#pragma unroll 1
+            for (int col = m.D + l.TK + 1; col < l.NC16; ++col) { QBT[tq + col * 4] = 0.0f; QDT[tq + col * 4] = 0.0f; }
+        }
+        // ---- q, qd: transposed operands; qd also as A of the first product (TMEM columns [0, DP8)).  The radial rows of qd
+        //      (the first n_R) are not stored anywhere: qd_n = sum_{T', k} cR[t][T'][n][k] Bd_k[T'], formed by the chunk's owner ----
+#pragma unroll 1
+        for (int c = h; 8 * c < l.DP8; c += NT) {
+            float qv[8], qd[8];
+            load_rows<8>(qp, 8 * c, m.D, qv);
+            load_rows<8>(qdp, 8 * c, m.D, qd);
+            if (c < nrc) {
+                float s[8];
 #pragma unroll
-            for (int c = 0; c < 2; ++c) {
-                if (r0 + 8 * c < l.DP8) {
-                    float hi[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        hi[j] = tf32_rn(qd[8 * c + j]);
-                        if (r0 + 8 * c + j < m.D) {
-                            QDT[tq + (r0 + 8 * c + j) * 4] = hi[j];
-                            QBT[tq + (r0 + 8 * c + j) * 4] = tf32_rn(qv[8 * c + j]);
-                        }
+                for (int j = 0; j < 8; ++j) s[j] = 0.0f;
+#pragma unroll 8
+                for (int r = 0; r < l.TK; ++r) {
+                    const float bdr = Bdp != nullptr ? __ldg(Bdp + (size_t)r * WARP) : 0.0f;
+                    const float* cr = sm + l.ocR + r * l.nR4 + 8 * c;          // nR4 >= 8 c + 4: the second quad only if it exists
+                    const float4 c0 = *reinterpret_cast<const float4*>(cr);
+                    s[0] = fmaf(c0.x, bdr, s[0]); s[1] = fmaf(c0.y, bdr, s[1]); s[2] = fmaf(c0.z, bdr, s[2]); s[3] = fmaf(c0.w, bdr, s[3]);
+                    if (8 * c + 4 < l.nR4) {
+                        const float4 c1 = *reinterpret_cast<const float4*>(cr + 4);
+                        s[4] = fmaf(c1.x, bdr, s[4]); s[5] = fmaf(c1.y, bdr, s[5]); s[6] = fmaf(c1.z, bdr, s[6]); s[7] = fmaf(c1.w, bdr, s[7]);
                     }
-                    tmem_st8(tb + r0 + 8 * c, hi);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    if (8 * c + j < m.nR) qd[j] = s[j];
+            }
+            float hi[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                hi[j] = tf32_rn(qd[j]);
+                if (8 * c + j < m.D) {
+                    QDT[tq + (8 * c + j) * 4] = hi[j];
+                    QBT[tq + (8 * c + j) * 4] = tf32_rn(qv[j]);
                 }
             }
-        };
-#pragma unroll
-        for (int cc = 0; cc < 2; ++cc) {
-            if (16 * cc < l.DP8) {
-                float qv[16], qd[16];
-                load_rows<16>(qp, 16 * cc, m.D, qv);
-                load_rows<16>(qdp, 16 * cc, m.D, qd);
-#pragma unroll
-                for (int j = 0; j < 16; ++j)
-                    if (16 * cc + j < 24 && 16 * cc + j < m.nR) qd[j] = qdr[(16 * cc + j) % 24];
-                put16(16 * cc, qv, qd);
-            }
-        }
-        #pragma unroll 1
-        for (int r0 = 32; r0 < l.DP8; r0 += 16) {
-            float qv[16], qd[16];
-            load_rows<16>(qp, r0, m.D, qv);
-            load_rows<16>(qdp, r0, m.D, qd);
-            put16(r0, qv, qd);
+            tmem_st8(tb + 8 * c, hi);
         }
         tmem_st_wait();
         fence_async_smem();
@@ -478,9 +502,9 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
         mbar_wait(mbar, phase); phase ^= 1;
         fence_after();
         // ---- gamma, e: A of the second product (TMEM [0, HP8)) and transposed operands; g_w1 ----
-        const float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TC_TM + tid;
-        #pragma unroll 1
-        for (int c0 = 0; c0 < l.HP8; c0 += 8) {
+        const float* hb = a.b.hbuf + (size_t)tile * l.HP8 * TC_TM + am;
+#pragma unroll 1
+        for (int c0 = 8 * h; c0 < l.HP8; c0 += 8 * NT) {
             float hh[8], xd[8], gam[8], om[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) hh[j] = hb[(size_t)(c0 + j) * TC_TM];
@@ -488,11 +512,11 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
             tmem_ld_wait();
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const float h = hh[j], w1 = sm[l.ow1 + c0 + j];
-                const float omh2 = fmaf(-h, h, 1.0f);
+                const float hv = hh[j], w1 = sm[l.ow1 + c0 + j];
+                const float omh2 = fmaf(-hv, hv, 1.0f);
                 const float e = valid ? w1 * omh2 : 0.0f;
-                const float g = fmaf(epsi, e, -2.0f * h * e * xd[j]);
-                om[j] = valid ? fmaf(epsi, h, omh2 * xd[j]) : 0.0f;
+                const float g = fmaf(epsi, e, -2.0f * hv * e * xd[j]);
+                om[j] = valid ? fmaf(epsi, hv, omh2 * xd[j]) : 0.0f;
                 gam[j] = tf32_rn(g);
                 GT[tg + (c0 + j) * 4] = gam[j];
                 ET[tg + (c0 + j) * 4] = tf32_rn(e);
@@ -509,16 +533,16 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
         if (tid == 0) {
             fence_after();
             tc_gemm_ts(tcol0 + l.cR2, tcol0, sm + l.oW2H, l.DP16, l.HP8, idesc2, false);     // Qb = Gamma W0s
-            // ACC (+)= GT^T-major products over the 128 atoms of the tile
+            // ACC (+)= products over the 128 atoms of the tile (K-major over atoms)
             const uint32_t d = tcol0 + l.cACC;
             const uint32_t gA = smem_u32(GT), eA = smem_u32(ET), qB = smem_u32(QBT), dB = smem_u32(QDT);
             bool acc = acc_live;
-            #pragma unroll 1
+#pragma unroll 1
             for (int k0 = 0; k0 < TC_TM; k0 += 8) {
                 mma_ss(d, make_desc(gA + (k0 >> 2) * l.ldG * 16, l.ldG * 16, 128), make_desc(qB + (k0 >> 2) * l.ldQ * 16, l.ldQ * 16, 128), idesc3, acc);
                 acc = true;
             }
-            #pragma unroll 1
+#pragma unroll 1
             for (int k0 = 0; k0 < TC_TM; k0 += 8)
                 mma_ss(d, make_desc(eA + (k0 >> 2) * l.ldG * 16, l.ldG * 16, 128), make_desc(dB + (k0 >> 2) * l.ldQ * 16, l.ldQ * 16, 128), idesc3, true);
             commit(mbar);
@@ -528,8 +552,8 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
         fence_after();
         // ---- Qb: only the angular rows are read later (the radial ones enter g_cR through ACC) ----
         float* qbp = valid ? sb_ptr(a.b.Qb, ib >> 5, m.D, ib & 31) : nullptr;
-        #pragma unroll 1
-        for (int c0 = (m.nR >> 3) << 3; c0 < l.DP8; c0 += 8) {
+#pragma unroll 1
+        for (int c0 = 8 * ((m.nR >> 3) + h); c0 < l.DP8; c0 += 8 * NT) {
             float f[8];
             tmem_ld8(tb + l.cR2 + c0, f);
             tmem_ld_wait();
@@ -542,7 +566,7 @@ __global__ void __launch_bounds__(TC_TM) k_ann_bwd_tc(StepArgs a, TcLay l)
     }
     if (acc_live) flush(cur_t);
     __syncthreads();
-    if (w == 0) tmem_dealloc(tcol0, l.ncols);
+    if (threadIdx.x < 32) tmem_dealloc(tcol0, l.ncols);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -553,14 +577,12 @@ bool ann_tc_fits(const nep_ctx* c, bool bwd)
     const ModelDev& m = c->m;
     if (m.H > 128 || m.D > 128 || m.nR > 24 || m.D + m.T * m.KR + 1 > 256) return false;
     const TcLay l = tc_layout(m, bwd);
-    // two blocks per SM or the FFMA tiles: one 128-thread block leaves the SM with four warps to cover the latencies of a tile
-    // (measured: config 4, one block per SM, k_ann_bwd 373 us against 295 us on the FFMA tiles)
-    return 2 * l.ncols <= 512 && 2 * (4 * (size_t)l.total + 1024) <= 228 * 1024;
+    return l.ncols <= 512 && 4 * (size_t)l.total <= (size_t)c->max_smem_optin;
 }
 
 // Persistent grid: blocks resident per SM by registers, shared memory and the 512 TMEM columns they share.  (The runtime's
 // occupancy calculator answers 1 for a kernel that allocates tensor memory, so the limits are worked out here.)
-static int tc_grid(nep_ctx* c, const void* kern, const TcLay& l, size_t smem, int* grid)
+static int tc_occupancy(nep_ctx* c, const void* kern, const TcLay& l, size_t smem, int threads, int* occ)
 {
     NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     cudaFuncAttributes fa;
@@ -569,32 +591,40 @@ static int tc_grid(nep_ctx* c, const void* kern, const TcLay& l, size_t smem, in
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
-    const int by_regs = regs_sm / (rup(std::max(fa.numRegs, 1), 8) * TC_TM);
+    const int by_regs = regs_sm / (rup(std::max(fa.numRegs, 1), 8) * threads);
     const int by_smem = (int)((size_t)smem_sm / (smem + fa.sharedSizeBytes + 1024));
-    const int occ = std::max(1, std::min(std::min(by_regs, by_smem), 512 / l.ncols));
-    *grid = std::min(c->b.ntiles, occ * c->sm_count);
+    const int by_thr = 2048 / threads;
+    *occ = std::max(1, std::min(std::min(std::min(by_regs, by_smem), by_thr), 512 / l.ncols));
+    return NEP_OK;
+}
+
+// two threads per atom when two blocks fit on an SM, four when only one does: sixteen warps per SM either way
+template <class K2, class K4>
+static int tc_launch(nep_ctx* c, const StepArgs& a, const TcLay& l, const char* name, K2 k2, K4 k4)
+{
+    const size_t smem = 4 * (size_t)l.total;
+    int occ2 = 1, occ4 = 1, rc;
+    if ((rc = tc_occupancy(c, (const void*)k2, l, smem, 2 * TC_TM, &occ2))) return rc;
+    if (occ2 >= 2) {
+        const int grid = std::min(c->b.ntiles, occ2 * c->sm_count);
+        NEP_LAUNCH(c, name, k2, grid, 2 * TC_TM, smem, a, l);
+    } else {
+        if ((rc = tc_occupancy(c, (const void*)k4, l, smem, 4 * TC_TM, &occ4))) return rc;
+        const int grid = std::min(c->b.ntiles, occ4 * c->sm_count);
+        NEP_LAUNCH(c, name, k4, grid, 4 * TC_TM, smem, a, l);
+    }
     return NEP_OK;
 }
 
 int launch_ann_fwd_tc(nep_ctx* c, const StepArgs& a)
 {
     if (c->b.ntiles == 0) return NEP_OK;
-    const TcLay l = tc_layout(c->m, false);
-    const size_t smem = 4 * (size_t)l.total;
-    int grid, rc;
-    if ((rc = tc_grid(c, (const void*)k_ann_fwd_tc, l, smem, &grid))) return rc;
-    NEP_LAUNCH(c, "k_ann_fwd", k_ann_fwd_tc, grid, TC_TM, smem, a, l);
-    return NEP_OK;
+    return tc_launch(c, a, tc_layout(c->m, false), "k_ann_fwd", k_ann_fwd_tc<2>, k_ann_fwd_tc<4>);
 }
 int launch_ann_bwd_tc(nep_ctx* c, const StepArgs& a)
 {
     if (c->b.ntiles == 0) return NEP_OK;
-    const TcLay l = tc_layout(c->m, true);
-    const size_t smem = 4 * (size_t)l.total;
-    int grid, rc;
-    if ((rc = tc_grid(c, (const void*)k_ann_bwd_tc, l, smem, &grid))) return rc;
-    NEP_LAUNCH(c, "k_ann_bwd", k_ann_bwd_tc, grid, TC_TM, smem, a, l);
-    return NEP_OK;
+    return tc_launch(c, a, tc_layout(c->m, true), "k_ann_bwd", k_ann_bwd_tc<2>, k_ann_bwd_tc<4>);
 }
 
 }  // namespace nep
