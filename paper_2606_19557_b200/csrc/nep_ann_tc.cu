@@ -600,12 +600,12 @@ static int tc_occupancy(nep_ctx* c, const void* kern, const TcLay& l, size_t sme
 
 // two threads per atom when two blocks fit on an SM, four when only one does: sixteen warps per SM either way
 template <class K2, class K4>
-static int tc_launch(nep_ctx* c, const StepArgs& a, const TcLay& l, const char* name, K2 k2, K4 k4)
+static int tc_launch(nep_ctx* c, const StepArgs& a, const TcLay& l, const char* name, K2 k2, K4 k4, bool prefer4)
 {
     const size_t smem = 4 * (size_t)l.total;
     int occ2 = 1, occ4 = 1, rc;
     if ((rc = tc_occupancy(c, (const void*)k2, l, smem, 2 * TC_TM, &occ2))) return rc;
-    if (occ2 >= 2) {
+    if (occ2 >= 2 && !prefer4) {
         const int grid = std::min(c->b.ntiles, occ2 * c->sm_count);
         NEP_LAUNCH(c, name, k2, grid, 2 * TC_TM, smem, a, l);
     } else {
@@ -619,12 +619,13 @@ static int tc_launch(nep_ctx* c, const StepArgs& a, const TcLay& l, const char* 
 int launch_ann_fwd_tc(nep_ctx* c, const StepArgs& a)
 {
     if (c->b.ntiles == 0) return NEP_OK;
-    return tc_launch(c, a, tc_layout(c->m, false), "k_ann_fwd", k_ann_fwd_tc<2>, k_ann_fwd_tc<4>);
+    // larger networks: four threads per atom also in the forward kernel (config 3, 50 x 37: 39 -> 34 us; config 2, 30 x 35: 28 -> 30)
+    return tc_launch(c, a, tc_layout(c->m, false), "k_ann_fwd", k_ann_fwd_tc<2>, k_ann_fwd_tc<4>, c->m.H * c->m.D > 1500);
 }
 int launch_ann_bwd_tc(nep_ctx* c, const StepArgs& a)
 {
     if (c->b.ntiles == 0) return NEP_OK;
-    return tc_launch(c, a, tc_layout(c->m, true), "k_ann_bwd", k_ann_bwd_tc<2>, k_ann_bwd_tc<4>);
+    return tc_launch(c, a, tc_layout(c->m, true), "k_ann_bwd", k_ann_bwd_tc<2>, k_ann_bwd_tc<4>, false);
 }
 
 }  // namespace nep

@@ -517,7 +517,7 @@ static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64
         c->cap_Sb = Sb;
     }
     if (!b.lacc) {   // loss accumulators and the block ticket: zero once, the loss kernel re-arms them itself
-        ALLOC(c, b.lacc, double, 8); ALLOC(c, b.counter, unsigned, 64);
+        ALLOC(c, b.lacc, double, 8 + 4 * 2 * (size_t)c->sm_count); ALLOC(c, b.counter, unsigned, 64);
         NEP_CUDA(c, cudaMemsetAsync(b.lacc, 0, 64, c->stream));
         NEP_CUDA(c, cudaMemsetAsync(b.counter, 0, 256, c->stream));
     }

@@ -22,7 +22,6 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
     for (int64_t ia = gid; ia < a.b.NBP; ia += nthreads) {
         const int w = (int)(ia >> 5), lane = (int)(ia & 31);
         const int4 bi = __ldg(a.b.binfo + w);
-        const bool valid = __ldg(a.d.type_p + (size_t)bi.x * WARP + lane) >= 0;
         const float c = (float)(2.0 * dlamF / (3.0 * a.b.nrmN));
         const float* Fp = sb_ptr(a.b.F, w, 3, lane);
         const float* Fl = sb_ptr(a.d.Flab, bi.x, 3, lane);
@@ -30,53 +29,66 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
         float s2 = 0.0f;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const float dF = valid ? Fp[k * WARP] - __ldg(Fl + k * WARP) : 0.0f;
+            const float dF = Fp[k * WARP] - __ldg(Fl + k * WARP);   // padding slots hold 0 in both (no type lookup on this path)
             s2 = fmaf(dF, dF, s2);
             up[k * WARP] = c * dF;
         }
         sF += (double)s2;
     }
+    // one fp64 division per structure (1 / N_s): a chain of ~40 of them per thread was the critical path of this kernel
+    const double cE = a.b.nrmS > 0.0 ? 2.0 * dlamE / a.b.nrmS : 0.0, cV = a.b.nrmV > 0.0 ? 2.0 * dlamV / (9.0 * a.b.nrmV) : 0.0;
     for (int sb = gid; sb < a.b.Sb; sb += nthreads) {
         const int sid = a.b.bsid[sb];
         const double n = (double)a.b.bnat[sb];
+        const double rn = 1.0 / n, rn2 = rn * rn;
         const double dE = a.b.Es[sb] - a.d.Elab[sid];
-        sE += (dE / n) * (dE / n);                                                  // Eq. 5
-        const float eps = (float)(2.0 * dlamE * dE / (a.b.nrmS * n * n));
+        sE += dE * dE * rn2;                                                        // Eq. 5
+        const float eps = (float)(cE * dE * rn2);
         a.b.eps[sb] = eps;
         sB += (double)eps * n;
         const bool hv = a.d.hasv[sid] != 0;
 #pragma unroll
         for (int k = 0; k < 9; ++k) {
             const double t = hv ? (double)a.b.Ws[9 * sb + k] - (double)a.d.Wlab[9 * (size_t)sid + k] : 0.0;
-            sW += (t / n) * (t / n);                                                // Eq. 7
-            a.b.G[9 * sb + k] = (hv && a.b.nrmV > 0.0) ? (float)(2.0 * dlamV * t / (9.0 * a.b.nrmV * n * n)) : 0.0f;
+            sW += t * t * rn2;                                                      // Eq. 7
+            a.b.G[9 * sb + k] = hv ? (float)(cV * t * rn2) : 0.0f;
         }
     }
-    // block reduction -> one atomic per block and quantity
+    // block reduction -> the block's four partial sums go to its own slot (no same-address floating-point atomics: a few
+    // hundred of those on one address cost ~10 us); the last block to finish (ticket) adds the slots in a fixed order
     __shared__ double red[4][8];
     __shared__ bool last;
     sF = warp_sum(sF); sE = warp_sum(sE); sW = warp_sum(sW); sB = warp_sum(sB);
     const int wid = threadIdx.x >> 5;
     if ((threadIdx.x & 31) == 0) { red[0][wid] = sE; red[1][wid] = sF; red[2][wid] = sW; red[3][wid] = sB; }
     __syncthreads();
+    double* part = a.b.lacc + 8;                 // [gridDim.x][4]
     if (threadIdx.x < 4) {
         double s = 0.0;
         for (int w = 0; w < 8; ++w) s += red[threadIdx.x][w];
-        if (s != 0.0) atomicAdd(a.b.lacc + threadIdx.x, s);
+        part[4 * blockIdx.x + threadIdx.x] = s;
     }
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) last = (atomicAdd(a.b.counter, 1u) == gridDim.x - 1);
     __syncthreads();
-    if (last && threadIdx.x == 0) {
+    if (last) {
         __threadfence();
-        volatile double* l = a.b.lacc;
-        const double dE = a.b.nrmS > 0.0 ? l[0] / a.b.nrmS : 0.0, dF = a.b.nrmN > 0.0 ? l[1] / (3.0 * a.b.nrmN) : 0.0, dV = a.b.nrmV > 0.0 ? l[2] / (9.0 * a.b.nrmV) : 0.0;
-        const double sb1 = l[3];
-        l[4] = dlamE * dE + dlamF * dF + dlamV * dV; l[5] = dE; l[6] = dF; l[7] = dV;   // Eq. 4
-        a.g[a.m.o_b1] = (float)(-sb1);                                                   // g_b1 = -sum_i eps_s(i)
-        l[0] = 0.0; l[1] = 0.0; l[2] = 0.0; l[3] = 0.0;
-        *a.b.counter = 0u;
+        if (wid < 4) {                           // warp q sums quantity q over the blocks
+            double s = 0.0;
+            for (unsigned b = threadIdx.x & 31; b < gridDim.x; b += 32) s += __ldcg(part + 4 * b + wid);
+            s = warp_sum(s);
+            if ((threadIdx.x & 31) == 0) red[wid][0] = s;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double* l = a.b.lacc;
+            const double dE = a.b.nrmS > 0.0 ? red[0][0] / a.b.nrmS : 0.0, dF = a.b.nrmN > 0.0 ? red[1][0] / (3.0 * a.b.nrmN) : 0.0,
+                         dV = a.b.nrmV > 0.0 ? red[2][0] / (9.0 * a.b.nrmV) : 0.0;
+            l[4] = dlamE * dE + dlamF * dF + dlamV * dV; l[5] = dE; l[6] = dF; l[7] = dV;   // Eq. 4
+            a.g[a.m.o_b1] = (float)(-red[3][0]);                                             // g_b1 = -sum_i eps_s(i)
+            *a.b.counter = 0u;
+        }
     }
 }
 
