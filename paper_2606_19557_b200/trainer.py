@@ -112,9 +112,13 @@ class Trainer:
         nb = 0
         for ids in epoch_batches(nep.n_struct, cfg.batch, cfg.seed, epoch):
             nep.set_batch(ids)
-            nep.forward_device()
-            sums += nep.loss_grad(spec.lambda_e, spec.lambda_f, spec.lambda_v, fetch_loss=True)
-            nep.adam_step(lr, variant=cfg.adam_variant)
+            if hasattr(nep, "train_step"):     # one call per step (a CUDA graph launch when a batch repeats)
+                nep.train_step(spec.lambda_e, spec.lambda_f, spec.lambda_v, lr, variant=cfg.adam_variant)
+                sums += nep.get_loss()
+            else:
+                nep.forward_device()
+                sums += nep.loss_grad(spec.lambda_e, spec.lambda_f, spec.lambda_v, fetch_loss=True)
+                nep.adam_step(lr, variant=cfg.adam_variant)
             nb += 1
         mean = sums / max(nb, 1)
         self._sched.step(float(mean[0]))          # takes effect from the next epoch (Eq. 14)
@@ -129,19 +133,22 @@ class Trainer:
                 callback(rec)
         return self.history
 
-    def rmse(self, n_atoms: Sequence[int], E: np.ndarray, F: np.ndarray, W: np.ndarray, chunk: int = 1024) -> dict:
-        """Root-mean-square errors over the whole loaded set: energy and virial per atom, force per component."""
+    def rmse(self, n_atoms: Sequence[int], has_virial: Optional[Sequence[int]] = None, chunk: int = 1024) -> dict:
+        """Root-mean-square errors over the whole loaded set: energy and virial per atom, force per component.
+
+        RMSE = sqrt(Delta) with the mean squares Delta_E, Delta_F, Delta_V of Eqs. 5-7 (P:69-73), which nep_loss_grad returns;
+        the set is evaluated in chunks of structures whose Deltas are recombined with their counts (S_b, N_b and the number
+        of structures with virial labels).  No arithmetic of Eqs. 5-7 is repeated here."""
         nep = self.nep
         n_atoms = np.asarray(n_atoms, dtype=np.int64)
-        off = np.concatenate([[0], np.cumsum(n_atoms)])
-        se = sf = sv = 0.0
+        hv = np.ones(len(n_atoms), dtype=np.int64) if has_virial is None else np.asarray(has_virial, dtype=np.int64)
+        wE = wF = wV = 0.0
         for i in range(0, nep.n_struct, chunk):
             ids = np.arange(i, min(i + chunk, nep.n_struct), dtype=np.int32)
             nep.set_batch(ids)
-            Eg, Fg, Wg = nep.forward()
-            n = n_atoms[ids].astype(np.float64)
-            se += float(np.sum(((Eg - E[ids]) / n) ** 2))
-            sv += float(np.sum(((Wg - W[ids]) / n[:, None]) ** 2))
-            sf += float(np.sum((Fg - F[off[ids[0]]:off[ids[-1] + 1]]) ** 2))
-        S, N = nep.n_struct, int(n_atoms.sum())
-        return {"energy_per_atom": (se / S) ** 0.5, "force": (sf / (3 * N)) ** 0.5, "virial_per_atom": (sv / (9 * S)) ** 0.5}
+            nep.forward_device()
+            _, dE, dF, dV = nep.loss_grad(1.0, 1.0, 1.0, fetch_loss=True)
+            wE += dE * len(ids); wF += dF * int(n_atoms[ids].sum()); wV += dV * int(hv[ids].sum())
+        S, N, Sv = nep.n_struct, int(n_atoms.sum()), int(hv.sum())
+        return {"energy_per_atom": (wE / max(S, 1)) ** 0.5, "force": (wF / max(N, 1)) ** 0.5,
+                "virial_per_atom": (wV / Sv) ** 0.5 if Sv else 0.0}

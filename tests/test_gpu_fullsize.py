@@ -20,10 +20,13 @@ def _draw(model, data, seed):
     return pd.network((q * s).mean(axis=0)).copy(), s
 
 
-@pytest.mark.parametrize("cfg", [2, 3, 4])
+@pytest.mark.parametrize("cfg", [2, 3, 4, "5 smallest model", "5 largest model"])
 def test_full_size_batch_against_oracle(cfg):
     from paper_2606_19557_b200.binding import Nep
-    w = wl.make_config(cfg)
+    if isinstance(cfg, str):          # config 5: the two ends of the model-complexity sweep (n_max 4 / 8, basis 8 / 12, 30 / 100 neurons)
+        w = wl.make_config(5, model=wl.config5_sweep()[0 if "smallest" in cfg else -1])
+    else:
+        w = wl.make_config(cfg)
     st = w.structures
     batch = wl.batches(w)[0]
     assert len(batch) == w.batch_size

@@ -72,6 +72,28 @@ def test_two_stage_switch_and_rate_constant_within_epoch():
     assert per_epoch[0] == {((1.0, 100.0, 1.0), 1e-2)} and per_epoch[4] == {((100.0, 5.0, 30.0), 1e-3)}
 
 
+def test_rmse_recombines_chunks_with_their_counts():
+    """Trainer.rmse over unequal chunks and a virial mask = sqrt of Eqs. 5-7 over the whole set (oracle-backed stand-in context:
+    the chunk bookkeeping is host logic)."""
+    from tests._oracle_nep import OracleNep
+    w = wl.tiny_workload(11, n_species=2, sizes=(5, 9, 3, 7, 6, 4), box=(3.4, 4.3, 3.1, 3.9, 3.6, 4.0))
+    prob = H.make_problem(w)
+    st = w.structures
+    hv = np.array([1, 0, 1, 1, 1, 0], np.uint8)
+    nep = OracleNep(w.model)
+    nep.load_structure_set(st, prob.E, prob.F, prob.W, hv)
+    nep.build_neighbors()
+    th = prob.theta + 0.05 * np.random.default_rng(0).normal(size=prob.theta.size)      # away from the teacher: non-zero errors
+    nep.set_params(th); nep.set_scaler(prob.scaler)
+    r = T.Trainer(nep, T.TrainConfig()).rmse(st.n_atoms, has_virial=hv, chunk=4)            # chunks of 4 and 2 structures
+    prob.data.set_labels(prob.E, prob.F, prob.W, hv)
+    l4, _ = O.loss_grad(prob.data, nep.theta, prob.scaler, (1.0, 1.0, 1.0), want_grad=False)
+    assert r["energy_per_atom"] == pytest.approx(np.sqrt(l4[1]), rel=1e-12)
+    assert r["force"] == pytest.approx(np.sqrt(l4[2]), rel=1e-12)
+    assert r["virial_per_atom"] == pytest.approx(np.sqrt(l4[3]), rel=1e-12)
+    assert min(r.values()) > 0
+
+
 @pytest.mark.gpu
 def test_trajectory_matches_oracle_and_loss_decreases():
     w = wl.make_config(1)
@@ -104,5 +126,16 @@ def test_trajectory_matches_oracle_and_loss_decreases():
         tr2 = T.Trainer(nep, cfg2)
         h2 = tr2.fit()
         assert h2[-1].loss < 0.2 * h2[0].loss, (h2[0].loss, h2[-1].loss)
-        r = tr2.rmse(st.n_atoms, prob.E, prob.F, prob.W)
-        assert set(r) == {"energy_per_atom", "force", "virial_per_atom"} and all(np.isfinite(x) and x >= 0 for x in r.values())
+        # RMSE report = sqrt of the mean squares of Eqs. 5-7 over the whole set, against the oracle at the trained parameters
+        hv = (np.arange(st.n_struct) % 3 != 1).astype(np.uint8)
+        nep.set_labels(prob.E, prob.F, prob.W, hv)
+        r = tr2.rmse(st.n_atoms, has_virial=hv, chunk=3)                 # three chunks of unequal size (3, 3, 2)
+        prob.data.set_labels(prob.E, prob.F, prob.W, hv)
+        try:
+            l4o, _ = O.loss_grad(prob.data, nep.get_params().astype(np.float64), prob.scaler, (1.0, 1.0, 1.0), want_grad=False)
+        finally:
+            prob.data.set_labels(prob.E, prob.F, prob.W)
+        assert r["energy_per_atom"] == pytest.approx(np.sqrt(l4o[1]), rel=2e-3)
+        assert r["force"] == pytest.approx(np.sqrt(l4o[2]), rel=1e-3)
+        assert r["virial_per_atom"] == pytest.approx(np.sqrt(l4o[3]), rel=1e-3)
+        assert r["force"] > 0 and r["virial_per_atom"] > 0
