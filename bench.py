@@ -45,10 +45,20 @@ def parse_args():
     return ap.parse_args()
 
 
-def make_workload(args, rank: int = 0):
+def make_workload(args, world: int = 1):
+    """The config's workload; data-parallel runs (weak scaling) take a `world` times longer prefix of the same seeded stream of
+    structures and a `world` times larger batch: every rank ends up with about one config's worth of DIFFERENT structures."""
+    import dataclasses
     from paper_2606_19557_b200 import workloads as wl
     model = wl.config5_sweep()[args.model_index] if args.config == 5 else None
-    return wl.make_config(args.config, n_struct=args.n_struct, model=model)
+    if world == 1:
+        return wl.make_config(args.config, n_struct=args.n_struct, model=model)
+    base = wl.make_config(args.config, n_struct=1, model=model)
+    S = args.n_struct if args.n_struct is not None else wl._CONFIGS[args.config]["n_struct"]
+    w = wl.make_config(args.config, n_struct=world * S, model=model)
+    B = min(wl._CONFIGS[args.config]["batch"], S)
+    del base
+    return dataclasses.replace(w, batch_size=world * B)
 
 
 def workload_name(w, args):
@@ -144,15 +154,60 @@ def setup_ours(w, stream=None):
     return nep, dict(load_s=t1 - t0, neighbors_cache_s=t2 - t1, params_labels_s=time.time() - t2)
 
 
-DP = {"world": 1, "views": None}   # data-parallel state of this process (world > 1: every rank holds one copy of the
-                                    # config's structures as its share of a `world` times larger set and batch)
+DP = {"world": 1, "views": None, "dpn": None}   # data-parallel state of this process: dpn = dataparallel.DataParallelNep holding
+                                                 # this rank's shard of the structures (sharded by structure, LPT on atoms)
 
 
-def dp_whole_batch(nep):
-    """Eqs. 5-7 divide by the counts of the WHOLE batch = world x this rank's (every rank runs the same shapes)."""
-    if DP["world"] > 1 or DP["views"] is not None:
-        Sb, Nb = nep.batch_shape()
-        nep.set_batch_normalisers(DP["world"] * Sb, DP["world"] * Nb, DP["world"] * Sb)
+def draw_theta_dp(dpn, model, seed):
+    """draw_theta over a sharded set: Eq. 2's ranges and the mean of the scaled descriptors are taken over every rank's atoms."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_19557_b200.workloads import ParamDraw
+    nep = dpn.nep
+    pd = ParamDraw(model, seed)
+    nep.set_params(pd.coefficients().astype(np.float32))
+    dpn.compute_scaler()                       # local ranges -> MIN / MAX all-reduce -> the same scaler on every rank
+    s = nep.get_scaler()
+    nep.forward(want=())
+    q = nep.get_descriptors().astype(np.float64)
+    acc = torch.tensor(np.concatenate([(q * s).sum(axis=0), [float(len(q))]]), device="cuda", dtype=torch.float64)
+    dist.all_reduce(acc)
+    acc = acc.cpu().numpy()
+    theta = pd.network(acc[:-1] / max(acc[-1], 1.0)).astype(np.float32)
+    return theta, s
+
+
+def setup_dp(w, rank, world):
+    """Every rank loads ITS shard of the `world` x larger set, builds its own lists and computes its own teacher labels."""
+    import torch
+    from paper_2606_19557_b200.dataparallel import DataParallelNep
+    t0 = time.time()
+    dpn = DataParallelNep(w.model, w.structures, rank, world)
+    st_local = w.structures.subset(dpn.shard.global_ids)
+    dpn.nep.load_structure_set(st_local)
+    t1 = time.time()
+    dpn.nep.build_neighbors()
+    dpn.nep.synchronize()
+    t2 = time.time()
+    nep = dpn.nep
+    th_t, s_t = draw_theta_dp(dpn, w.model, w.seeds["teacher"])
+    nep.set_params(th_t); nep.set_scaler(s_t)
+    nep.set_batch(None)
+    E, F, W = nep.forward()
+    nep.set_labels(E.astype(np.float64), F.astype(np.float64), W.astype(np.float64))
+    th_s, s_s = draw_theta_dp(dpn, w.model, w.seeds["student"])
+    nep.set_params(th_s); nep.set_scaler(s_s)
+    torch.cuda.synchronize()
+    return dpn, dict(load_s=t1 - t0, neighbors_cache_s=t2 - t1, params_labels_s=time.time() - t2)
+
+
+def set_batch_ids(nep, ids):
+    """Selects a batch given by GLOBAL structure ids (None = every structure): through the shard table when data-parallel."""
+    dpn = DP["dpn"]
+    if dpn is None:
+        nep.set_batch(ids)
+    else:
+        dpn.set_batch(np.arange(len(dpn.n_atoms), dtype=np.int32) if ids is None else ids)   # local part + whole-batch normalisers
 
 
 def dp_exchange(nep):
@@ -177,8 +232,7 @@ def one_step(nep, lam, graph=False):
 def e2e_step(nep, lam, ids):
     """The call sequence a user makes per training step, HOST buffers in and out: the batch's structure ids go in
     (nep_set_batch copies them and the slice tables to the device), the loss comes back (nep_loss_grad -> host)."""
-    nep.set_batch(ids)
-    dp_whole_batch(nep)
+    set_batch_ids(nep, ids)
     if DP["views"] is None:
         nep.train_step(lam[0], lam[1], lam[2], LR, use_graph=True)   # one graph launch (captured again when the batch's shape changes)
         return nep.get_loss()                      # the step's loss terms -> host
@@ -212,12 +266,15 @@ def run_ours(args):
         nbuild.build()
     if use_dist:
         dist.barrier()
-    w = make_workload(args, rank)
-    nep, setup = setup_ours(w)
+    w = make_workload(args, world)
     lam = w.lambdas
     DP["world"] = world
     if use_dist:
+        DP["dpn"], setup = setup_dp(w, rank, world)
+        nep = DP["dpn"].nep
         DP["views"] = nep.grad_loss_tensors()
+    else:
+        nep, setup = setup_ours(w)
     blist = wl.batches(w)
     full_batches = [b for b in blist if len(b) == w.batch_size] or blist
     single = len(blist) == 1
@@ -229,13 +286,11 @@ def run_ours(args):
 
     def set_b(i):
         if not single:
-            nep.set_batch(full_batches[i % len(full_batches)])
-            dp_whole_batch(nep)
+            set_batch_ids(nep, full_batches[i % len(full_batches)])
 
     # ---- warm-up ----
     if single:
-        nep.set_batch(None)
-        dp_whole_batch(nep)
+        set_batch_ids(nep, None)
     for i in range(max(args.warmup, 3)):
         set_b(i); one_step(nep, lam, graph=i % 2 == 1)
     torch.cuda.synchronize()
@@ -248,9 +303,6 @@ def run_ours(args):
         dist.barrier()
     torch.cuda.synchronize()
     clocks = ClockSampler(local) if rank == 0 else None
-    nep.profile_enable(True)
-    PROF_EVERY = 5          # per-kernel CUDA events on every 5th timed step (event records between kernels cost ~10 % of a step)
-    n_prof = 0
     l0 = nep.launch_count()
     t0 = time.time()
     for i in range(K):
@@ -259,20 +311,27 @@ def run_ours(args):
             flush.fill_(i & 0xFF)
         sz = nep.batch_shape()
         structs += sz[0]; atoms += sz[1]
-        sampled = i % PROF_EVERY == 0
-        nep.profile_pause(not sampled)
-        n_prof += int(sampled)
         ev[i][0].record()
-        one_step(nep, lam, graph=not sampled)      # sampled steps: the three calls, with CUDA events between their kernels
+        one_step(nep, lam, graph=True)
         ev[i][1].record()
     torch.cuda.synchronize()
     t1 = time.time()
     if world > 1:
         dist.barrier()
     launches = nep.launch_count() - l0
+    clk = clocks.stop(t0, t1) if clocks else None
+    # ---- per-kernel times: a separate pass of steps through the three calls with CUDA events around every kernel (the event
+    #      records between kernels cost ~10 % of a step, so they stay out of the timed region) ----
+    n_prof = max(4, K // 5)
+    nep.profile_enable(True)
+    for i in range(n_prof):
+        set_b(i)
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        one_step(nep, lam, graph=False)
+    torch.cuda.synchronize()
     prof = nep.profile_read()
     nep.profile_enable(False)
-    clk = clocks.stop(t0, t1) if clocks else None
     ms_steps = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(ms_steps))
     if world > 1:
@@ -315,6 +374,8 @@ def run_ours(args):
     te1 = time.perf_counter()
     for i in range(K):                                            # bookkeeping of what the K steps moved, outside the clock
         ids = e2e_batches[i % len(e2e_batches)]
+        if DP["dpn"] is not None:                                 # this rank's part of the batch
+            ids = DP["dpn"].shard.global_ids[DP["dpn"].shard.local_batch(ids)]
         e_atoms += int(w.structures.n_atoms[ids].sum())
         nbs = int(np.sum((w.structures.n_atoms[ids] + 31) // 32))
         h2d += nbs * 16 + len(ids) * (16 + 4 * w.model.n_species)   # slice table, structure tables (nep_set_batch)
@@ -333,10 +394,7 @@ def run_ours(args):
         dist.destroy_process_group()
         return
     # ---- roofline of the dominant kernel ----
-    if single:
-        nep.set_batch(None)
-    else:
-        nep.set_batch(full_batches[0])
+    set_batch_ids(nep, None if single else full_batches[0])
     sizes = nep.get_sizes()
     models = rf.kernel_models(w.model, sizes)
     ksum = sum(v[0] for v in prof.values())
@@ -347,7 +405,7 @@ def run_ours(args):
     mdl = models.get(top)
     roof = None
     if mdl:
-        dur = kern[top]["ms"] * 1e-3
+        dur = kern[top]["ms"] * kern[top]["launches_per_step"] * 1e-3     # the work model is per step
         t_alu, t_hbm = mdl["flops"] / alu_peak, mdl["bytes"] / (hbm_peak * 1e9)
         if t_alu >= t_hbm:
             roof = {"kernel": top, "bound": "alu", "achieved": mdl["flops"] / dur / 1e12, "peak": alu_peak / 1e12, "unit": "TFLOP/s",
@@ -356,12 +414,14 @@ def run_ours(args):
             roof = {"kernel": top, "bound": "hbm", "achieved": mdl["bytes"] / dur / 1e9, "peak": hbm_peak, "unit": "GB/s", "peak_source": peak_src}
         roof["frac"] = roof["achieved"] / roof["peak"]
         roof["traffic"] = None
-        tpath = os.path.join(ROOT, "profiles", "r01d_traffic.json")   # DRAM bytes per launch from the committed ncu capture
+        tpath = os.path.join(ROOT, "profiles", "r02_traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
         if os.path.exists(tpath):
             tj = json.load(open(tpath))
-            if tj.get("workload") == f"config{w.config_id}" and args.n_struct is None:
+            if tj.get("csrc_sha") != rf.csrc_hash():
+                roof["traffic_source"] = "none: the kernel sources changed after the capture in profiles/r02_traffic.json"
+            elif tj.get("workload") == f"config{w.config_id}" and args.n_struct is None and world == 1:
                 roof["traffic"] = tj["bytes_per_launch"].get(top)
-                roof["traffic_source"] = "profiles/r01d_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
+                roof["traffic_source"] = tj.get("source", "profiles/r02_summary.md") + " (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
         roof["share_of_step"] = kern[top]["share"]
         roof["avg_ms"] = kern[top]["ms"]
         roof["algorithmic_flops_per_launch"] = mdl["flops"]
@@ -376,16 +436,21 @@ def run_ours(args):
                    "atoms_per_step": atoms // K // world, "pairs_R_per_step": sizes["P_R_b"], "pairs_A_per_step": sizes["P_A_b"],
                    "l2": ("flushed between timed steps (256 MB write)" if flush is not None else "not flushed; per-step working set exceeds L2"),
                    "ms_per_step_back_to_back_no_flush": ms_b2b, "ms_per_step_back_to_back_three_calls": ms_b2b_stream,
-                   "step_call": "nep_train_step (one CUDA graph launch per step; every 5th timed step runs nep_forward + nep_loss_grad + nep_adam_step with per-kernel CUDA events)", "kernel_events": f"every {PROF_EVERY}th timed step ({n_prof} of {K})", "setup_s": setup,
-                   "device_bytes": nep.bytes_allocated, "parallelism": (f"dp{world}: structures sharded, whole batch = {world} x {w.batch_size} structures, one NCCL all-reduce of g "
-                                    f"[{w.model.n_par} fp32] + 4 loss terms per step" if use_dist else "dp1 (one GPU, no collective)")},
+                   "step_call": ("nep_train_step: one CUDA graph launch per step" if not use_dist else "nep_forward + nep_loss_grad + all-reduce + nep_adam_step"),
+                   "kernel_events": f"{n_prof} extra steps after the timed region, through the three calls with CUDA events around every kernel", "setup_s": setup,
+                   "device_bytes": nep.bytes_allocated, "parallelism": (f"dp{world}: {w.structures.n_struct} structures sharded by structure over the ranks (dataparallel.DataParallelNep: "
+                                    f"each rank holds different ones), whole batch = {w.batch_size} structures, scaler from a MIN / MAX all-reduce, "
+                                    f"one NCCL all-reduce of g [{w.model.n_par} fp32] + 4 loss terms per step" if use_dist else "dp1 (one GPU, no collective)")},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
                 "what": "per step: nep_set_batch(host ids) + nep_train_step (one graph launch) + nep_get_loss(-> host); geometry cache resident (P:143)"},
         "gpu_launches": int(launches),
         "clocks": clk,
         "roofline": roof,
-        "kernels": {k: {"avg_ms": round(v["ms"], 5), "share": round(v["share"], 4), "per_step": v["launches_per_step"]} for k, v in
-                    sorted(kern.items(), key=lambda kv: -kv[1]["share"])},
+        "kernels": {k: dict({"avg_ms": round(v["ms"], 5), "share": round(v["share"], 4), "per_step": v["launches_per_step"]},
+                            **({"frac_alu": round(models[k]["flops"] / alu_peak / (v["ms"] * v["launches_per_step"] * 1e-3), 4),
+                                "frac_hbm": round(models[k]["bytes"] / (hbm_peak * 1e9) / (v["ms"] * v["launches_per_step"] * 1e-3), 4)}
+                               if k in models and v["ms"] > 0 else {}))
+                    for k, v in sorted(kern.items(), key=lambda kv: -kv[1]["share"])},
         "step_model": {"flops": tot["flops"], "bytes": tot["bytes"], "alu_frac_of_step": tot["flops"] / alu_peak / (ms_step * 1e-3),
                        "hbm_frac_of_step": tot["bytes"] / (hbm_peak * 1e9) / (ms_step * 1e-3)},
     }

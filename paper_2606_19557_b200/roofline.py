@@ -63,5 +63,19 @@ def fp32_peak_flops(sm_count: int = 148, sm_mhz: float = 1965.0, lanes: int = 12
     return sm_count * lanes * 2 * sm_mhz * 1e6
 
 
+def csrc_hash() -> str:
+    """SHA-256 (first 16 hex digits) over the kernel sources: a stored ncu figure is only quoted for the kernels it measured."""
+    import hashlib
+    import os
+    d = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def step_totals(models: dict) -> dict:
     return {"flops": sum(v["flops"] for v in models.values()), "bytes": sum(v["bytes"] for v in models.values())}
