@@ -104,7 +104,7 @@ class Nep:
     """One context = one CUDA device + one stream (include/nep.h).  Method names are the C calls without `nep_`."""
 
     def __init__(self, n_species: int, rc_R: float, rc_A: float, n_max_R: int, n_max_A: int, basis_R: int, basis_A: int,
-                 l_max_3b: int = 4, l_max_4b: int = 2, l_max_5b: int = 1, neurons: int = 30, stream=None):
+                 l_max_3b: int = 4, l_max_4b: int = 2, l_max_5b: int = 1, neurons: int = 30, stream=None, guard_bytes: int = 0):
         import torch
         self._L = load_library()
         self._h = C.c_void_p(None)
@@ -113,6 +113,11 @@ class Nep:
         self._torch = torch
         self._bufs = {}
         self.bytes_allocated = 0
+        # debugging aid (compute-sanitizer is not available everywhere): every device buffer handed to the library gets a guard
+        # band of `guard_bytes` (a multiple of 256) filled with 0xA5 on both sides; check_guards() verifies they are untouched
+        self._guard = int(guard_bytes)
+        if self._guard % 256:
+            raise ValueError("guard_bytes must be a multiple of 256")
         if stream is None:
             stream = torch.cuda.current_stream()
         self.stream = stream
@@ -122,11 +127,16 @@ class Nep:
                 # allocate on the stream the library launches on: the caching allocator then reuses a freed block only
                 # in that stream's order, whatever torch's current stream is when the callback runs
                 with torch.cuda.stream(self.stream):
-                    t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda")
+                    t = torch.empty(int(nbytes) + 2 * self._guard, dtype=torch.uint8, device="cuda")
+                    if self._guard:
+                        t[:self._guard].fill_(0xA5); t[self._guard + int(nbytes):].fill_(0xA5)
             except Exception:      # noqa: BLE001  (OOM -> NULL -> NEP_ENOMEM)
                 return None
-            p = t.data_ptr()
-            self._bufs[p] = t
+            p = t.data_ptr() + self._guard
+            self._bufs[p] = t[self._guard:self._guard + int(nbytes)] if self._guard else t
+            if self._guard:
+                self._guarded = getattr(self, "_guarded", {})
+                self._guarded[p] = (t, int(nbytes))
             self.bytes_allocated += int(nbytes)
             return p
 
@@ -134,6 +144,8 @@ class Nep:
             t = self._bufs.pop(p, None)
             if t is not None:
                 self.bytes_allocated -= t.numel()
+            if self._guard and p in getattr(self, "_guarded", {}):
+                self._freed_ok = getattr(self, "_freed_ok", True) and self._bands_intact(*self._guarded.pop(p))
 
         self._alloc_cb = ALLOC_FN(_alloc)
         self._free_cb = FREE_FN(_free)
@@ -147,6 +159,22 @@ class Nep:
         self.n_par = int(self._L.nep_num_params(h))
         self.n_struct = 0
         self.n_atoms_total = 0
+
+    def _bands_intact(self, t, nbytes) -> bool:
+        g = self._guard
+        return bool((t[:g] == 0xA5).all().item()) and bool((t[g + nbytes:] == 0xA5).all().item())
+
+    def check_guards(self) -> int:
+        """Number of live buffers whose guard bands were verified; raises if a band was written (also for buffers already freed)."""
+        self._torch.cuda.synchronize()
+        if not self._guard:
+            raise RuntimeError("context was created without guard_bytes")
+        if not getattr(self, "_freed_ok", True):
+            raise RuntimeError("a guard band of a buffer that has since been released was overwritten")
+        bad = [hex(p) for p, (t, n) in getattr(self, "_guarded", {}).items() if not self._bands_intact(t, n)]
+        if bad:
+            raise RuntimeError(f"guard bands overwritten next to {len(bad)} device buffers: {bad[:4]}")
+        return len(getattr(self, "_guarded", {}))
 
     @classmethod
     def from_model(cls, model, **kw) -> "Nep":

@@ -425,6 +425,17 @@ __global__ void __launch_bounds__(TC_TM * NT) k_ann_bwd_tc(StepArgs a, TcLay l)
         }
         const int ib = a.b.alist[(size_t)tile * TC_TM + am];
         const bool valid = ib >= 0;
+        if (tile + 1 < tile1 && h == 0) {
+            // the rows of the next tile -> L2 while this one is worked on: per 32-atom slice they are contiguous blocks
+            const int ib2 = a.b.alist[(size_t)(tile + 1) * TC_TM + am];
+            if (ib2 >= 0 && ((ib2 & 31) == 0 || lane == 0)) {
+                const size_t ws2 = (size_t)(ib2 >> 5);
+                prefetch_l2(a.b.q + ws2 * m.D * WARP, 4u * m.D * WARP);
+                prefetch_l2(a.b.qd + ws2 * m.D * WARP, 4u * m.D * WARP);
+                prefetch_l2(a.b.Bd + ws2 * l.TK * WARP, 4u * l.TK * WARP);
+            }
+            if (tid == 0) prefetch_l2(a.b.hbuf + (size_t)(tile + 1) * l.HP8 * TC_TM, 4u * l.HP8 * TC_TM);
+        }
         const float *qp = nullptr, *qdp = nullptr, *Bp = nullptr, *Bdp = nullptr;
         float epsi = 0.0f;
         if (valid) {
