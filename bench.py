@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--model-index", type=int, default=0, help="config 5: which of the 8 sweep models")
+    ap.add_argument("--sustain", type=float, default=0.0, help="also run steps back to back for this many seconds with the clocks sampled")
     return ap.parse_args()
 
 
@@ -357,6 +358,22 @@ def run_ours(args):
     b.record(); torch.cuda.synchronize()
     ms_b2b_stream = a.elapsed_time(b) / K
 
+    # ---- sustained: seconds of back-to-back steps under the power cap, clocks and power sampled (the timed region above is short) ----
+    sustained = None
+    if args.sustain > 0 and rank == 0 and world == 1:
+        cs = ClockSampler(local, period_ms=200)
+        n_done = 0
+        ts0 = time.time()
+        a.record()
+        while time.time() - ts0 < args.sustain:
+            for i in range(200):
+                set_b(n_done + i); one_step(nep, lam, graph=True)
+            n_done += 200
+            torch.cuda.synchronize()
+        b.record(); torch.cuda.synchronize()
+        ts1 = time.time()
+        sustained = {"seconds": ts1 - ts0, "steps": n_done, "ms_per_step": a.elapsed_time(b) / n_done, "clocks": cs.stop(ts0, ts1)}
+
     # ---- e2e: host ids in, host loss out, every step ----
     e2e_batches = full_batches if not single else [np.arange(w.structures.n_struct, dtype=np.int32)]
     for i in range(3):
@@ -454,6 +471,8 @@ def run_ours(args):
         "step_model": {"flops": tot["flops"], "bytes": tot["bytes"], "alu_frac_of_step": tot["flops"] / alu_peak / (ms_step * 1e-3),
                        "hbm_frac_of_step": tot["bytes"] / (hbm_peak * 1e9) / (ms_step * 1e-3)},
     }
+    if sustained is not None:
+        out["sustained"] = sustained
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(args, w, seconds_target=15.0)
     nep.destroy()
