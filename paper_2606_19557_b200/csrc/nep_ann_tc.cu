@@ -133,10 +133,13 @@ __device__ __forceinline__ float tanh_fast(float x)
 // issue the K loop of one product: D (+)= A[tmem cols acol ..] B[smem, [K/4][rows][4]]
 __device__ __forceinline__ void tc_gemm_ts(uint32_t d, uint32_t acol, const float* B, int rows, int K, uint32_t idesc, bool acc)
 {
-    const uint32_t b0 = smem_u32(B);
+    // the descriptor of K step k0 + 8 is the previous one with the start-address field (16-byte units) advanced by two K chunks
+    uint64_t bd = make_desc(smem_u32(B), rows * 16, 128);
+    const uint64_t step = (uint64_t)(2 * rows);
 #pragma unroll 1
     for (int k0 = 0; k0 < K; k0 += 8) {
-        mma_ts(d, acol + k0, make_desc(b0 + (k0 >> 2) * rows * 16, rows * 16, 128), idesc, acc);
+        mma_ts(d, acol + k0, bd, idesc, acc);
+        bd += step;
         acc = true;
     }
 }
@@ -364,6 +367,7 @@ __global__ void __launch_bounds__(TC_TM * NT) k_ann_bwd_tc(StepArgs a, TcLay l)
     int cur_t = -1;
     bool acc_live = false;                        // ACC holds sums of the current species
     float* gw1s = sm + l.ogw1;                    // [HP8] g_w1 of the current species, summed over this block's atoms
+    int ib_next = tile0 < tile1 ? a.b.alist[(size_t)tile0 * TC_TM + am] : -1;   // atom of the tile to come (loaded one tile ahead)
     float* QBT = sm + l.oQBT; float* QDT = sm + l.oQDT; float* GT = sm + l.oGT; float* ET = sm + l.oET;
     const int tq = ((am >> 2) * l.ldQ) * 4 + (am & 3), tg = ((am >> 2) * l.ldG) * 4 + (am & 3);   // this atom's cell of row 0
     const int nrc = (m.nR + 7) >> 3;              // chunks of qd that hold radial rows
@@ -423,11 +427,12 @@ __global__ void __launch_bounds__(TC_TM * NT) k_ann_bwd_tc(StepArgs a, TcLay l)
             }
             __syncthreads();                       // cRt is read below before the next barrier
         }
-        const int ib = a.b.alist[(size_t)tile * TC_TM + am];
+        const int ib = ib_next;
         const bool valid = ib >= 0;
+        ib_next = tile + 1 < tile1 ? a.b.alist[(size_t)(tile + 1) * TC_TM + am] : -1;
         if (tile + 1 < tile1 && h == 0) {
             // the rows of the next tile -> L2 while this one is worked on: per 32-atom slice they are contiguous blocks
-            const int ib2 = a.b.alist[(size_t)(tile + 1) * TC_TM + am];
+            const int ib2 = ib_next;
             if (ib2 >= 0 && ((ib2 & 31) == 0 || lane == 0)) {
                 const size_t ws2 = (size_t)(ib2 >> 5);
                 prefetch_l2(a.b.q + ws2 * m.D * WARP, 4u * m.D * WARP);
@@ -548,14 +553,20 @@ __global__ void __launch_bounds__(TC_TM * NT) k_ann_bwd_tc(StepArgs a, TcLay l)
             const uint32_t d = tcol0 + l.cACC;
             const uint32_t gA = smem_u32(GT), eA = smem_u32(ET), qB = smem_u32(QBT), dB = smem_u32(QDT);
             bool acc = acc_live;
-#pragma unroll 1
+            const uint64_t sA = (uint64_t)(2 * l.ldG), sB = (uint64_t)(2 * l.ldQ);     // two K chunks, in 16-byte units of the address field
+            uint64_t ad = make_desc(gA, l.ldG * 16, 128), bd = make_desc(qB, l.ldQ * 16, 128);
+#pragma unroll 4
             for (int k0 = 0; k0 < TC_TM; k0 += 8) {
-                mma_ss(d, make_desc(gA + (k0 >> 2) * l.ldG * 16, l.ldG * 16, 128), make_desc(qB + (k0 >> 2) * l.ldQ * 16, l.ldQ * 16, 128), idesc3, acc);
+                mma_ss(d, ad, bd, idesc3, acc);
+                ad += sA; bd += sB;
                 acc = true;
             }
-#pragma unroll 1
-            for (int k0 = 0; k0 < TC_TM; k0 += 8)
-                mma_ss(d, make_desc(eA + (k0 >> 2) * l.ldG * 16, l.ldG * 16, 128), make_desc(dB + (k0 >> 2) * l.ldQ * 16, l.ldQ * 16, 128), idesc3, true);
+            ad = make_desc(eA, l.ldG * 16, 128); bd = make_desc(dB, l.ldQ * 16, 128);
+#pragma unroll 4
+            for (int k0 = 0; k0 < TC_TM; k0 += 8) {
+                mma_ss(d, ad, bd, idesc3, true);
+                ad += sA; bd += sB;
+            }
             commit(mbar);
         }
         acc_live = true;
