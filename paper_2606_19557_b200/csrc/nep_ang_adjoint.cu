@@ -1,53 +1,37 @@
 // nep_ang_adjoint.cu -- S9: the adjoint sweep giving the gradient of the angular descriptor coefficients (DESIGN C12)
 //   g_cA[ti][tj][n][k] += [sum_L Sb_nL b_L + sum_L EdS_nL (grad b_L . d~)] f_k + [sum_L EdS_nL b_L] (r^.d~) f_k'
-// The two terms need different per-atom tensors in registers (Sb = J^T Qb + Fp H Sd, and EdS = dE_i/dS), so they are
-// two PASSES over the pair records.  A thread accumulates acc[n][k] for its run of one neighbour type (records are
-// sorted by neighbour type).  One species: a block runs both passes and shuffle-reduces the accumulators.
-//
-// Several species (blockIdx.z = pass): reduction over atoms without votes, atomics or read-modify-write chains inside the sweep: when a lane's run of
-// neighbour type t_j ends it stores its accumulators into its own COLUMN of a table
-// tab[warp][(t_j, n, k)][column] (row stride 33 words: the per-lane stores and the per-row reads are both conflict
-// free).  Columns are the lanes of the warp sorted by centre type t_i, so after the sweep the sum over the atoms of
-// one (t_i, t_j) is a sum over a contiguous column range: the threads of the block each own a few rows, walk the
-// 32 columns once and issue one RED per (t_i, t_j, n, k) and block.  Types a lane never met are zero-filled by
-// that lane after its sweep.
+// The two terms need different per-atom tensors in registers (Sb = J^T Qb + HS, and EdS = dE_i/dS), so they are two PASSES over
+// the pair records.  A thread accumulates acc[n][k] over its pairs.
+// One species (k_ang_adjoint): a block runs both passes and shuffle-reduces the accumulators; the per-atom rows of the second pass
+// are requested into shared memory before the first pass starts (rows_request), those of the first pass are loaded branch free.
+// Several species (k_ang_adjoint_ms): one warp per block and pass, snapshot table (below).
 #include <algorithm>
 
 #include "nep_kernels.cuh"
 
 namespace nep {
 
-constexpr int ADJ_TST = WARP + 1;   // table row stride (words)
-
-// MULTI = false (one species): both passes in one block, shuffle reduction of the accumulators at the end.
-// MULTI = true: blockIdx.z selects the pass; per-lane columns in the shared-memory table.
-template <int NCH, int K, bool MULTI>
+template <int NCH, int K, bool STAGED>
 __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
 {
     extern __shared__ __align__(16) float smem[];
     const ModelDev& m = a.m;
-    constexpr int NK = NCH * K;
+    constexpr int NK = NCH * K, NKP = (NK + 3) & ~3;
     const int nwarp = blockDim.x >> 5;
-    const int T = m.T, rows = T * NK;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
-    float* tab_all = smem + PAIR_TB * 16;                                           // MULTI: [nwarp][rows][ADJ_TST]; else [nwarp][NK]
-    int* cend_all = reinterpret_cast<int*>(tab_all + (size_t)nwarp * rows * ADJ_TST);   // MULTI: [nwarp][T] end column of each centre type
+    float* tab_all = smem + PAIR_TB * 16;                                           // [nwarp][NK]
     const int n0 = blockIdx.y * NCH;
     const int wib = threadIdx.x >> 5;
+    float* area = tab_all + (size_t)nwarp * NKP + (size_t)wib * staged_warp_floats(m, NCH);
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(tab_all + (size_t)nwarp * NKP + (size_t)nwarp * staged_warp_floats(m, NCH)) + wib;
+    if (STAGED) {   // rows of pass 1, on their way while pass 0 runs
+        const size_t w = (size_t)blockIdx.x * nwarp + wib;
+        if (w < (size_t)a.b.nbs)
+            rows_request(mbar, area, a.b.S + (w * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
+                         area + NCH * NL * WARP, a.b.Fp + (w * m.D + m.nR) * WARP, m.D - m.nR);
+    }
     Lane L;
     const bool inb = lane_init(a, L);
-    if (!inb) L.ti = -1;
-    // MULTI: column of this lane = its rank among the lanes of the warp sorted by centre type (padding lanes: none)
-    int col = 0;
-    if (MULTI) {
-        int base = 0;
-        for (int t = 0; t < T; ++t) {
-            const unsigned bm = __ballot_sync(0xffffffffu, L.ti == t);
-            if (L.ti == t) col = base + __popc(bm & ((1u << (threadIdx.x & 31)) - 1u));
-            base += __popc(bm);
-            if ((threadIdx.x & 31) == 0) cend_all[wib * T + t] = base;
-        }
-    }
     constexpr int KH = (K + 1) / 2;
     float2 acc2[NCH][KH];   // (acc_n,2i, acc_n,2i+1); the odd tail pairs with a zero basis value
 #pragma unroll
@@ -55,53 +39,18 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
 #pragma unroll
         for (int k = 0; k < KH; ++k) acc2[n][k] = make_float2(0.0f, 0.0f);
     auto accv = [&](int n, int k) -> float& { return (k & 1) ? acc2[n][k >> 1].y : acc2[n][k >> 1].x; };
-    if (inb && L.ti >= 0) {
-        float* tab = tab_all + (size_t)wib * rows * ADJ_TST + col;
+    if (inb) {
         const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
-        int cur = -1;
-        unsigned seen = 0u;
-        // MULTI: end of this lane's run of neighbour type `cur`: accumulators -> own column of the table
-        auto store_run = [&]() {
-            float* c0 = tab + (size_t)cur * NK * ADJ_TST;
-#pragma unroll
-            for (int n = 0; n < NCH; ++n)
-#pragma unroll
-                for (int k = 0; k < K; ++k) { c0[(n * K + k) * ADJ_TST] = accv(n, k); accv(n, k) = 0.0f; }
-            seen |= 1u << cur;
-        };
-        auto next_type = [&](int tj) {
-            if (MULTI && tj != cur) {
-                if (cur >= 0) store_run();
-                cur = tj;
-            }
-        };
+        sweep2_begin<PAIR_TB>(sw.rec, sw.width, stage);
         const float rcinv = m.rcinvA;
         float2 X2[NCH][NL / 2];
-        if (!MULTI || blockIdx.z == 0) {
+        {
             // ---- pass 0: Sb ----
             {
                 float X[NCH][NL];
-                const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
-                const float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
-                const float* Qbp = sb_ptr(a.b.Qb, L.w, m.D, L.lane);
-                const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
+                load_Sbar<NCH>(a, L, n0, X);
 #pragma unroll
-                for (int n = 0; n < NCH; ++n) {
-                    if (n0 + n < m.nA) {
-                        float S[NL], Sd[NL], cq[6], cf[6];
-                        const size_t o = (size_t)(n0 + n) * NL * WARP;
-#pragma unroll
-                        for (int l = 0; l < NL; ++l) { S[l] = Sp[o + l * WARP]; Sd[l] = Sdp[o + l * WARP]; }
-                        load_inv_coef(m, Qbp, n0 + n, cq);
-                        load_inv_coef(m, Fpp, n0 + n, cf);
-                        inv_adjoint(S, cq, X[n]);
-                        inv_hessian_action(S, Sd, cf, X[n]);
-                    } else {
-#pragma unroll
-                        for (int l = 0; l < NL; ++l) X[n][l] = 0.0f;
-                    }
-                    pack24(X[n], X2[n]);
-                }
+                for (int n = 0; n < NCH; ++n) pack24(X[n], X2[n]);
             }
             struct Prep { PairGeo p; float fv[2 * KH]; };
             auto prep = [&](const float4& rc4, float on) {
@@ -130,17 +79,23 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                     for (int k = 0; k < KH; ++k) acc2[n][k] = __ffma2_rn(aa, make_float2(P.fv[2 * k], P.fv[2 * k + 1]), acc2[n][k]);
                 }
             };
-            sweep_pairs2<PAIR_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+            sweep2_run<PAIR_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
                 const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
                 contract(A);
                 contract(B);
             });
         }
-        if (!MULTI || blockIdx.z == 1) {
+        {
             // ---- pass 1: EdS ----
+            sweep2_begin<PAIR_TB>(sw.rec, sw.width, stage);
             {
                 float X[NCH][NL];
-                load_EdS<NCH>(a, L, n0, X);
+                if (STAGED) {
+                    rows_wait(mbar);
+                    load_EdS_staged<NCH>(m, L.ti, n0, area + L.lane, area + NCH * NL * WARP + L.lane, X);
+                } else {
+                    load_EdS<NCH>(a, L, n0, X);
+                }
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) pack24(X[n], X2[n]);
             }
@@ -184,62 +139,29 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                                                 __ffma2_rn(bb, make_float2(P.dfv[2 * k], P.dfv[2 * k + 1]), acc2[n][k]));
                 }
             };
-            sweep_pairs2<PAIR_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+            sweep2_run<PAIR_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
                 const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
                 contract(A);
                 contract(B);
             });
         }
-        if (MULTI) {
-            if (cur >= 0) store_run();
-            // neighbour types this atom never met: zeros
-            for (int tj = 0; tj < T; ++tj) {
-                if ((seen >> tj) & 1u) continue;
-                float* c0 = tab + (size_t)tj * NK * ADJ_TST;
+        // every lane targets the same block of coefficients -> shuffle-reduce, lane 0 stores, block adds
 #pragma unroll
-                for (int e = 0; e < NK; ++e) c0[e * ADJ_TST] = 0.0f;
+        for (int n = 0; n < NCH; ++n)
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const float v = warp_sum(accv(n, k));
+                if ((threadIdx.x & 31) == 0) tab_all[wib * NKP + n * K + k] = v;
             }
-        }
-    }
-    if (!MULTI) {
-        // one species: every lane targets the same block of coefficients -> shuffle-reduce, lane 0 stores, block adds
-        if (inb) {
-#pragma unroll
-            for (int n = 0; n < NCH; ++n)
-#pragma unroll
-                for (int k = 0; k < K; ++k) {
-                    const float v = warp_sum(accv(n, k));
-                    if ((threadIdx.x & 31) == 0) tab_all[wib * NK + n * K + k] = v;
-                }
-        } else {
-            for (int i = threadIdx.x & 31; i < NK; i += WARP) tab_all[wib * NK + i] = 0.0f;
-        }
-        __syncthreads();
-        for (int i = threadIdx.x; i < NK; i += blockDim.x) {
-            float v = 0.0f;
-            for (int w = 0; w < nwarp; ++w) v += tab_all[w * NK + i];
-            const int n = i / K, k = i - n * K;
-            if (v != 0.0f && k < m.KA && n0 + n < m.nA) atomicAdd(a.g + m.o_cA + (size_t)(n0 + n) * m.KA + k, v);
-        }
-        return;
+    } else {
+        for (int i = threadIdx.x & 31; i < NK; i += WARP) tab_all[wib * NKP + i] = 0.0f;
     }
     __syncthreads();
-    // thread owns rows r = (t_j, n, k); for each centre type the sum over its (contiguous) column range of every warp
-    for (int r = threadIdx.x; r < rows; r += blockDim.x) {
-        const int tj = r / NK, e = r - tj * NK, n = e / K, k = e - n * K;
-        if (!(k < m.KA && n0 + n < m.nA)) continue;
-        float* gp = a.g + m.o_cA + ((size_t)tj * m.nA + n0 + n) * m.KA + k;
-        const size_t tstep = (size_t)T * m.nA * m.KA;
-        for (int ti = 0; ti < T; ++ti) {
-            float v = 0.0f;
-            for (int w = 0; w < nwarp; ++w) {
-                const float* row = tab_all + ((size_t)w * rows + r) * ADJ_TST;
-                const int c0 = ti ? cend_all[w * T + ti - 1] : 0, c1 = cend_all[w * T + ti];
-#pragma unroll 4
-                for (int c = c0; c < c1; ++c) v += row[c];
-            }
-            if (v != 0.0f) atomicAdd(gp + ti * tstep, v);
-        }
+    for (int i = threadIdx.x; i < NK; i += blockDim.x) {
+        float v = 0.0f;
+        for (int w = 0; w < nwarp; ++w) v += tab_all[w * NKP + i];
+        const int n = i / K, k = i - n * K;
+        if (v != 0.0f && k < m.KA && n0 + n < m.nA) atomicAdd(a.g + m.o_cA + (size_t)(n0 + n) * m.KA + k, v);
     }
 }
 
@@ -296,27 +218,9 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
         if (blockIdx.z == 0) {
             {
                 float X[NCH][NL];
-                const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
-                const float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
-                const float* Qbp = sb_ptr(a.b.Qb, L.w, m.D, L.lane);
-                const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
+                load_Sbar<NCH>(a, L, n0, X);
 #pragma unroll
-                for (int n = 0; n < NCH; ++n) {
-                    if (n0 + n < m.nA) {
-                        float S[NL], Sd[NL], cq[6], cf[6];
-                        const size_t o = (size_t)(n0 + n) * NL * WARP;
-#pragma unroll
-                        for (int l = 0; l < NL; ++l) { S[l] = Sp[o + l * WARP]; Sd[l] = Sdp[o + l * WARP]; }
-                        load_inv_coef(m, Qbp, n0 + n, cq);
-                        load_inv_coef(m, Fpp, n0 + n, cf);
-                        inv_adjoint(S, cq, X[n]);
-                        inv_hessian_action(S, Sd, cf, X[n]);
-                    } else {
-#pragma unroll
-                        for (int l = 0; l < NL; ++l) X[n][l] = 0.0f;
-                    }
-                    pack24(X[n], X2[n]);
-                }
+                for (int n = 0; n < NCH; ++n) pack24(X[n], X2[n]);
             }
             sweep_pairs_tb<WARP>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& rc4) {
                 const PairGeo p = pair_geo(rc4);
@@ -431,8 +335,16 @@ int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
         constexpr int NK = NCH * K;
         if (m.T == 1) {
             const int nw = PAIR_TB / WARP;
-            const size_t smem = (size_t)PAIR_TB * 64 + 4 * (size_t)nw * NK;
-            NEP_LAUNCH(c, "k_ang_adjoint", (k_ang_adjoint<NCH, K, false>), dim3((unsigned)((c->b.nbs + nw - 1) / nw), a.nchunks), nw * WARP, smem, a);
+            const size_t base = (size_t)PAIR_TB * 64 + 4 * (size_t)nw * ((NK + 3) & ~3);
+            const size_t smem = base + 4 * nw * staged_warp_floats(m, NCH) + STAGED_BAR_BYTES;
+            const dim3 grid((unsigned)((c->b.nbs + nw - 1) / nw), a.nchunks);
+            if (2 * smem + 2048 <= (size_t)c->max_smem_sm) {
+                auto kern = k_ang_adjoint<NCH, K, true>;
+                if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                NEP_LAUNCH(c, "k_ang_adjoint", kern, grid, nw * WARP, smem, a);
+            } else {
+                NEP_LAUNCH(c, "k_ang_adjoint", (k_ang_adjoint<NCH, K, false>), grid, nw * WARP, base, a);
+            }
         } else {
             constexpr int NKP = (NK + 3) & ~3;
             const int LS = (m.T * NKP) + ((((m.T * NKP) >> 2) & 1) ? 0 : 4);

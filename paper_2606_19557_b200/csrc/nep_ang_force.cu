@@ -5,7 +5,9 @@
 
 namespace nep {
 
-template <int NCH, int K>
+// STAGED: the per-atom rows of the prologue (moments of the chunk, angular rows of Fp) come through shared memory (rows_request),
+// requested before the coefficient table is filled; otherwise (tables too large for that) they are loaded into registers directly.
+template <int NCH, int K, bool STAGED>
 __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
 {
     extern __shared__ __align__(16) float smem[];
@@ -14,15 +16,35 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
     float* cs = smem + SWEEP2_SMEM_BYTES / 4;
     const int n0 = blockIdx.y * NCH;
+    const int wib = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    float* area0 = cs + ((m.T * m.T * CST + 3) & ~3);
+    float* area = area0 + (size_t)wib * staged_warp_floats(m, NCH);
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(area0 + (size_t)nwarp * staged_warp_floats(m, NCH)) + wib;
+    if (STAGED) {
+        const size_t w = (size_t)blockIdx.x * nwarp + wib;
+        if (w < (size_t)a.b.nbs)
+            rows_request(mbar, area, a.b.S + (w * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
+                         area + NCH * NL * WARP, a.b.Fp + (w * m.D + m.nR) * WARP, m.D - m.nR);
+    }
+    Lane L;
+    const bool inb = lane_init(a, L);
+    SweepA sw;
+    if (inb) {
+        sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+        sweep2_begin<SWEEP2_TB>(sw.rec, sw.width, stage);
+    }
     load_cA_chunk<NCH, K>(a, cs, n0);
     __syncthreads();
-    Lane L;
-    if (!lane_init(a, L)) return;
-    const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+    if (!inb) return;
     float2 E2[NCH][NL / 2];   // dE_i/dS in packed pairs
     {
         float EdS[NCH][NL];
-        load_EdS<NCH>(a, L, n0, EdS);
+        if (STAGED) {
+            rows_wait(mbar);
+            load_EdS_staged<NCH>(m, L.ti, n0, area + L.lane, area + NCH * NL * WARP + L.lane, EdS);
+        } else {
+            load_EdS<NCH>(a, L, n0, EdS);
+        }
 #pragma unroll
         for (int n = 0; n < NCH; ++n) pack24(EdS[n], E2[n]);
     }
@@ -80,7 +102,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
         w[3] = fmaf(-p.dy, px, w[3]); w[4] = fmaf(-p.dy, py, w[4]); w[5] = fmaf(-p.dy, pz, w[5]);
         w[6] = fmaf(-p.dz, px, w[6]); w[7] = fmaf(-p.dz, py, w[7]); w[8] = fmaf(-p.dz, pz, w[8]);
     };
-    sweep_pairs2<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+    sweep2_run<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
         const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
         contract(A);
         if (has2) contract(B);
@@ -102,10 +124,17 @@ int launch_ang_force(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
-        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m);
-        auto kern = k_ang_force<NCH, K>;
-        if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        NEP_LAUNCH(c, "k_ang_force", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+        const size_t base = SWEEP2_SMEM_BYTES + ((cA_chunk_bytes<NCH, K>(m) + 15) & ~(size_t)15);
+        const size_t smem = base + 4 * (PAIR_TB / WARP) * staged_warp_floats(m, NCH) + STAGED_BAR_BYTES;
+        if (2 * smem + 2048 <= (size_t)c->max_smem_sm) {      // two blocks per SM (the register limit) keep fitting
+            auto kern = k_ang_force<NCH, K, true>;
+            if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            NEP_LAUNCH(c, "k_ang_force", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+        } else {
+            auto kern = k_ang_force<NCH, K, false>;
+            if (base > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
+            NEP_LAUNCH(c, "k_ang_force", kern, dim3(gx, a.nchunks), PAIR_TB, base, a);
+        }
     });
     return NEP_OK;
 }

@@ -7,7 +7,9 @@
 
 namespace nep {
 
-template <int NCH, int K>
+// STAGED: the rows of B that S1 reads are requested into shared memory before the pair sweep and S1 runs after it (the rows have
+// long arrived); otherwise S1 runs first, from global memory.
+template <int NCH, int K, bool STAGED>
 __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
 {
     extern __shared__ __align__(16) float smem[];
@@ -17,7 +19,19 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
     float* cs = smem + SWEEP2_SMEM_BYTES / 4;
     float* cR = cs + m.T * m.T * CST;                 // chunk 0 only: radial coefficients transposed to [ti][tj][k][n], n padded to 4
     const int nRP = (m.nR + 3) & ~3;
+    const int TK = m.T * m.KR;
+    const int wib = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    float* barea = cR + m.T * m.T * m.KR * nRP + (size_t)wib * TK * WARP;   // STAGED: this warp's rows of B
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(cR + m.T * m.T * m.KR * nRP + (size_t)nwarp * TK * WARP) + wib;
     const int n0 = blockIdx.y * NCH;
+    Lane L;
+    const bool inb = lane_init(a, L);
+    SweepA sw;
+    if (inb) {
+        if (STAGED && blockIdx.y == 0) rows_request(mbar, barea, a.d.B + (size_t)L.ds * TK * WARP, TK, nullptr, nullptr, 0);
+        sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
+        sweep2_begin<SWEEP2_TB>(sw.rec, sw.width, stage);
+    }
     load_cA_chunk<NCH, K>(a, cs, n0);
     if (blockIdx.y == 0)
 #pragma unroll 8
@@ -26,16 +40,11 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
             cR[i] = n < m.nR ? __ldg(a.theta + m.o_cR + (pt * m.nR + n) * m.KR + k) : 0.0f;
         }
     __syncthreads();
-    Lane L;
-    if (!lane_init(a, L)) return;
+    if (!inb) return;
     float* qp = sb_ptr(a.b.q, L.w, m.D, L.lane);
 
-    if (blockIdx.y == 0) {   // ---- S1 ----
-        // the structure accumulators that the force sweeps add into start from zero (benign duplicate stores)
-        if (L.lane < 9) a.b.Ws[9 * L.sb + L.lane] = 0.0f;
-        else if (L.lane == 9) a.b.Es[L.sb] = 0.0;
-        const float* Bp = sb_ptr(a.d.B, L.ds, m.T * m.KR, L.lane);
-        // q_n = sum_{T', k} cR[t_i][T'][n][k] B_k[T']: every B value is loaded once and meets 8 channels in registers
+    // ---- S1 ----  q_n = sum_{T', k} cR[t_i][T'][n][k] B_k[T']: every B value is loaded once and meets 8 channels in registers
+    auto radial_descriptors = [&](const float* Bp) {   // Bp: row 0 of B for this lane, rows WARP apart (global or staged)
         for (int n0 = 0; n0 < m.nR; n0 += 8) {
             float acc[8];
 #pragma unroll
@@ -43,11 +52,10 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
             if (L.ti >= 0) {
                 const bool two = n0 + 4 < nRP;
                 const float* cc = cR + (size_t)L.ti * m.T * m.KR * nRP + n0;   // rows r = T' * KR + k are nRP apart
-                const int TK = m.T * m.KR;
                 for (int r0 = 0; r0 < TK; r0 += 8) {
                     float b[8];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) b[j] = r0 + j < TK ? __ldg(Bp + (size_t)(r0 + j) * WARP) : 0.0f;   // eight loads in flight
+                    for (int j = 0; j < 8; ++j) b[j] = r0 + j < TK ? Bp[(size_t)(r0 + j) * WARP] : 0.0f;   // eight loads in flight
 #pragma unroll
                     for (int j = 0; j < 8; ++j)
                         if (r0 + j < TK) {
@@ -64,10 +72,15 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
             for (int j = 0; j < 8; ++j)
                 if (n0 + j < m.nR) qp[(size_t)(n0 + j) * WARP] = acc[j];
         }
+    };
+    if (blockIdx.y == 0) {
+        // the structure accumulators that the force sweeps add into start from zero (benign duplicate stores)
+        if (L.lane < 9) a.b.Ws[9 * L.sb + L.lane] = 0.0f;
+        else if (L.lane == 9) a.b.Es[L.sb] = 0.0;
+        if (!STAGED) radial_descriptors(sb_ptr(a.d.B, L.ds, TK, L.lane));
     }
 
     // ---- S2 ----
-    const SweepA sw = sweep_init(a.d.recoffA, a.d.recA, a.d.cntA, L);
     float2 S2[NCH][NL / 2];   // (S_n,2i, S_n,2i+1): accumulated with packed FFMA2 (one issue slot per two lanes' FMAs)
 #pragma unroll
     for (int n = 0; n < NCH; ++n)
@@ -95,11 +108,15 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
             for (int l = 0; l < NL / 2; ++l) S2[n][l] = __ffma2_rn(gg, make_float2(b[2 * l], b[2 * l + 1]), S2[n][l]);
         }
     };
-    sweep_pairs2<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
+    sweep2_run<SWEEP2_TB>(sw.rec, sw.width, sw.cnt, stage, [&](const float4& ra, const float4& rb, bool has2) {
         const Prep A = prep(ra, 1.0f), B = prep(rb, has2 ? 1.0f : 0.0f);
         accumulate(A);
         accumulate(B);
     });
+    if (STAGED && blockIdx.y == 0) {
+        rows_wait(mbar);
+        radial_descriptors(barea + L.lane);
+    }
     float S[NCH][NL];
 #pragma unroll
     for (int n = 0; n < NCH; ++n)
@@ -125,10 +142,17 @@ int launch_ang_fwd(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
-        const size_t smem = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.KR * ((m.nR + 3) & ~3));
-        auto kern = k_ang_fwd<NCH, K>;
-        if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        NEP_LAUNCH(c, "k_ang_fwd", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+        const size_t base = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.KR * ((m.nR + 3) & ~3));
+        const size_t smem = base + 4 * (size_t)(PAIR_TB / WARP) * m.T * m.KR * WARP + STAGED_BAR_BYTES;
+        if (3 * smem + 3072 <= (size_t)c->max_smem_sm) {      // three blocks per SM (the register limit) keep fitting
+            auto kern = k_ang_fwd<NCH, K, true>;
+            if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            NEP_LAUNCH(c, "k_ang_fwd", kern, dim3(gx, a.nchunks), PAIR_TB, smem, a);
+        } else {
+            auto kern = k_ang_fwd<NCH, K, false>;
+            if (base > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)base));
+            NEP_LAUNCH(c, "k_ang_fwd", kern, dim3(gx, a.nchunks), PAIR_TB, base, a);
+        }
     });
     return NEP_OK;
 }

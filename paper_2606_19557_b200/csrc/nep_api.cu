@@ -153,6 +153,7 @@ int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&c->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaDeviceGetAttribute(&c->max_smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     {   // network kernels: tensor-core tiles when they fit; NEP_ANN_FFMA=1 selects the FFMA tiles (measurement aid)
         const char* e = getenv("NEP_ANN_FFMA");
         c->ann_tc = !(e && e[0] == '1') && ann_tc_fits(c, false) && ann_tc_fits(c, true);

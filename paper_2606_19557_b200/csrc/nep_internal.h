@@ -119,7 +119,7 @@ struct nep_ctx {
     cudaStream_t stream;
     std::string err;
     std::vector<void*> allocs;
-    int sm_count; int max_smem_optin;
+    int sm_count; int max_smem_optin; int max_smem_sm;
     bool ann_tc = false;   // network kernels on tcgen05 (nep_ann_tc.cu) instead of the FFMA tiles (nep_ann.cu)
 
     // host copies of the data set

@@ -9,6 +9,7 @@
 #pragma once
 #include "nep_internal.h"
 #include "nep_math.cuh"
+#include "nep_umma.cuh"
 
 namespace nep {
 
@@ -194,8 +195,10 @@ __device__ __forceinline__ void sweep_pairs_tb(const float4* __restrict__ rec, i
 // stage: 4 staging cells per thread, SWEEP2_TB apart.
 constexpr int SWEEP2_TB = 128;
 constexpr int SWEEP2_SMEM_BYTES = SWEEP2_TB * 16 * 4;
-template <int TB, class Body2>
-__device__ __forceinline__ void sweep_pairs2(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body2&& body2)
+// sweep2_begin requests the first four slots (two groups); sweep2_run consumes the records.  They are separate so that a kernel can
+// compute its prologue while the records arrive.
+template <int TB>
+__device__ __forceinline__ void sweep2_begin(const float4* __restrict__ rec, int width, float4* stage)
 {
 #pragma unroll
     for (int g = 0; g < 2; ++g) {
@@ -204,6 +207,10 @@ __device__ __forceinline__ void sweep_pairs2(const float4* __restrict__ rec, int
             if (2 * g + h < width) cp_async16(stage + (2 * g + h) * TB, rec + (size_t)(2 * g + h) * WARP);
         cp_async_commit();
     }
+}
+template <int TB, class Body2>
+__device__ __forceinline__ void sweep2_run(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body2&& body2)
+{
     for (int s = 0; s < width; s += 2) {
         cp_async_wait<1>();
         float4* c0 = stage + (s & 3) * TB;
@@ -221,6 +228,41 @@ __device__ __forceinline__ void sweep_pairs2(const float4* __restrict__ rec, int
     }
     cp_async_wait<0>();
 }
+template <int TB, class Body2>
+__device__ __forceinline__ void sweep_pairs2(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body2&& body2)
+{
+    sweep2_begin<TB>(rec, width, stage);
+    sweep2_run<TB>(rec, width, cnt, stage, body2);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-atom rows through shared memory.  The prologue / epilogue of an angular sweep reads 120-300 slice-blocked rows per warp;
+// loaded channel after channel into registers they are 5-10 dependent DRAM round trips with little to overlap them at two
+// warps per scheduler (ncu, config 2: 27-35 % of a sweep's warp time sits there).  The rows of one slice are contiguous
+// (rows x 128 bytes), so lane 0 of the warp requests each block of rows with ONE bulk copy (cp.async.bulk, the TMA engine)
+// into the warp's own shared-memory area, as the first thing the kernel does (the addresses depend on the block index only);
+// completion is signalled on the warp's mbarrier, independent of the cp.async groups of the pair records, and awaited where the
+// rows are first needed.  Every lane then reads its column area[row * 32 + lane], conflict free.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* mbar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(umma::smem_u32(dst)), "l"(src), "r"(bytes), "r"(umma::smem_u32(mbar)) : "memory");
+}
+// whole warp calls; two blocks of rows (either may be empty).  rows_wait afterwards, by every lane, before the first read.
+__device__ __forceinline__ void rows_request(uint64_t* mbar, float* dst0, const float* src0, int rows0, float* dst1, const float* src1, int rows1)
+{
+    if ((threadIdx.x & 31) == 0) {
+        umma::mbar_init(mbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        const uint32_t b0 = (uint32_t)rows0 * (4 * WARP), b1 = (uint32_t)rows1 * (4 * WARP);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(umma::smem_u32(mbar)), "r"(b0 + b1) : "memory");
+        if (b0) bulk_g2s(dst0, src0, b0, mbar);
+        if (b1) bulk_g2s(dst1, src1, b1, mbar);
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ void rows_wait(uint64_t* mbar) { umma::mbar_wait(mbar, 0); }
 
 struct SweepA { const float4* rec; int width, cnt; };
 __device__ __forceinline__ SweepA sweep_init(const int64_t* __restrict__ recoff, const float4* __restrict__ recs,
@@ -328,28 +370,97 @@ __device__ __forceinline__ void unpack24(const float2* b2, float* b)
     for (int i = 0; i < NL / 2; ++i) { b[2 * i] = b2[i].x; b[2 * i + 1] = b2[i].y; }
 }
 
-// EdS_nL = dE_i/dS_nL = sum_a Fp[q index (a, n)] dq_a/dS_nL for the NCH channels of this thread (DESIGN C8)
+// EdS_nL = dE_i/dS_nL = sum_a Fp[q index (a, n)] dq_a/dS_nL for the NCH channels of this thread (DESIGN C8).
+// Branch free (channels beyond n_A and padding lanes read a valid row and select zero), so that the loads of all channels are
+// issued together: one DRAM round trip instead of one per channel.
 template <int NCH>
 __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n0, float (*EdS)[NL])
 {
     const ModelDev& m = a.m;
     const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
     const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
+    float S[NCH][NL], coef[NCH][6];
 #pragma unroll
     for (int n = 0; n < NCH; ++n) {
-        if (n0 + n < m.nA && L.ti >= 0) {
-            float S[NL], coef[6];
-            const float* sp = Sp + (size_t)(n0 + n) * NL * WARP;
+        const int nn = n0 + n < m.nA ? n0 + n : m.nA - 1;
+        const float* sp = Sp + (size_t)nn * NL * WARP;
 #pragma unroll
-            for (int l = 0; l < NL; ++l) S[l] = sp[l * WARP];
-            load_inv_coef(m, Fpp, n0 + n, coef);
-            inv_adjoint(S, coef, EdS[n]);
-        } else {
+        for (int l = 0; l < NL; ++l) S[n][l] = __ldg(sp + l * WARP);
 #pragma unroll
-            for (int l = 0; l < NL; ++l) EdS[n][l] = 0.0f;
-        }
+        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Fpp + (size_t)ang_row(m, s, nn) * WARP);
+        coef[n][4] = __ldg(Fpp + (size_t)ang_row(m, m.has4 ? 4 : 0, nn) * WARP);
+        coef[n][5] = __ldg(Fpp + (size_t)ang_row(m, m.has5 ? 5 : 0, nn) * WARP);
+    }
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        const bool ok = n0 + n < m.nA && L.ti >= 0;
+#pragma unroll
+        for (int s = 0; s < 4; ++s) coef[n][s] = ok ? coef[n][s] : 0.0f;
+        coef[n][4] = (ok && m.has4) ? coef[n][4] : 0.0f;
+        coef[n][5] = (ok && m.has5) ? coef[n][5] : 0.0f;
+        inv_adjoint(S[n], coef[n], EdS[n]);
     }
 }
+
+// Sb_nL = sum_a Qb[(a, n)] dq_a/dS_nL + HS_nL: the per-atom tensor of the first pass of the adjoint sweep (DESIGN C12); HS is the
+// second-derivative term that the tangent sweep left in b.Sd.  Branch free like load_EdS.
+template <int NCH>
+__device__ __forceinline__ void load_Sbar(const StepArgs& a, const Lane& L, int n0, float (*X)[NL])
+{
+    const ModelDev& m = a.m;
+    const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
+    const float* Hp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
+    const float* Qbp = sb_ptr(a.b.Qb, L.w, m.D, L.lane);
+    float S[NCH][NL], coef[NCH][6];
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        const int nn = n0 + n < m.nA ? n0 + n : m.nA - 1;
+        const float* sp = Sp + (size_t)nn * NL * WARP;
+        const float* hp = Hp + (size_t)nn * NL * WARP;
+#pragma unroll
+        for (int l = 0; l < NL; ++l) { S[n][l] = __ldg(sp + l * WARP); X[n][l] = __ldg(hp + l * WARP); }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Qbp + (size_t)ang_row(m, s, nn) * WARP);
+        coef[n][4] = __ldg(Qbp + (size_t)ang_row(m, m.has4 ? 4 : 0, nn) * WARP);
+        coef[n][5] = __ldg(Qbp + (size_t)ang_row(m, m.has5 ? 5 : 0, nn) * WARP);
+    }
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        const bool ok = n0 + n < m.nA && L.ti >= 0;
+#pragma unroll
+        for (int s = 0; s < 4; ++s) coef[n][s] = ok ? coef[n][s] : 0.0f;
+        coef[n][4] = (ok && m.has4) ? coef[n][4] : 0.0f;
+        coef[n][5] = (ok && m.has5) ? coef[n][5] : 0.0f;
+        float t[NL];
+        inv_adjoint(S[n], coef[n], t);
+#pragma unroll
+        for (int l = 0; l < NL; ++l) X[n][l] = ok ? t[l] + X[n][l] : 0.0f;
+    }
+}
+
+// The same from rows staged in shared memory: Ss = the NCH x 24 moment rows of the chunk, Fs = the angular rows nR .. D-1 of Fp
+// (both [row][lane], pointers at this lane's column).
+template <int NCH>
+__device__ __forceinline__ void load_EdS_staged(const ModelDev& m, int ti, int n0, const float* Ss, const float* Fs, float (*EdS)[NL])
+{
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        const bool ok = n0 + n < m.nA && ti >= 0;
+        const int nn = n0 + n < m.nA ? n0 + n : m.nA - 1;
+        float S[NL], coef[6];
+#pragma unroll
+        for (int l = 0; l < NL; ++l) S[l] = ok ? Ss[(n * NL + l) * WARP] : 0.0f;
+#pragma unroll
+        for (int s = 0; s < 4; ++s) coef[s] = ok ? Fs[(s * m.nA + nn) * WARP] : 0.0f;
+        coef[4] = (ok && m.has4) ? Fs[(4 * m.nA + nn) * WARP] : 0.0f;
+        coef[5] = (ok && m.has5) ? Fs[((4 + m.has4) * m.nA + nn) * WARP] : 0.0f;
+        inv_adjoint(S, coef, EdS[n]);
+    }
+}
+// rows of the chunk's moments and of the angular part of a [D]-row array, and the shared-memory floats a warp needs for both
+__device__ __forceinline__ int chunk_rows(const ModelDev& m, int n0, int nch) { return (m.nA - n0 < nch ? m.nA - n0 : nch) * NL; }
+__host__ __device__ inline size_t staged_warp_floats(const ModelDev& m, int nch) { return (size_t)(nch * NL + (m.D - m.nR)) * WARP; }
+constexpr size_t STAGED_BAR_BYTES = (PAIR_TB / WARP) * 8;   // one mbarrier per warp of a block, after the areas
 
 // d~ = u_i - u_j - G^T d ;  returns t = r^ . d~ and the tangent rho = (d~ - t r^) / r of r^
 struct Tangent { float t, rx, ry, rz; };
