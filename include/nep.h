@@ -59,13 +59,28 @@ typedef void (*nep_free_fn)(void* user, void* ptr);
 const char* nep_version(void);
 
 /* Model definition (Table I).  1 <= n_species <= 16 (the paper's largest set);
- * 0 < rc_A <= rc_R (DESIGN G22); n_max >= 0; 1 <= basis <= 16; l_max_3b == 4; l_max_4b in {0,2};
- * l_max_5b in {0,1} (Table I: "l_max 4 2 1"); neurons >= 1.
+ * 0 < rc_A <= rc_R (DESIGN G22); n_max >= 0; 1 <= basis <= 16; l_max_3b in 1..4 (three-body orders l = 1..l_max_3b;
+ * Table I uses 4); l_max_4b in {0,2}; l_max_5b in {0,1} (Table I: "l_max 4 2 1"); neurons >= 1.
  * cuda_stream: a cudaStream_t (NULL = default stream).  alloc/free_/alloc_user: see above.
  * On success *out owns the context; release with nep_destroy. */
 int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max_R, int n_max_A,
                int basis_R, int basis_A, int l_max_3b, int l_max_4b, int l_max_5b, int neurons,
                nep_alloc_fn alloc, nep_free_fn free_, void* alloc_user, void* cuda_stream);
+
+/* A model as a file, and prediction with it ("prediction").  nep_save_model writes the hyper-parameters of
+ * Table I, the scaler of Eq. 2 [D] and theta [N_par, layout of DESIGN C0] as text:
+ *     nep_b200_model 1 / n_species T / cutoff rc_R rc_A / n_max R A / basis_size R A / l_max l3 l4 l5 / neuron H /
+ *     scaler D, D values / theta N_par, N_par values (9 significant digits: fp32 values round-trip exactly).
+ * The keywords are those of the paper's input file (Table I); the layout is this library's own (the paper does not print the
+ * layout of GPUMD's model files, DESIGN reading G28).  Needs parameters and a scaler (NEP_ESTATE otherwise).
+ * nep_create_from_model_file = nep_create with the file's hyper-parameters + nep_set_params + nep_set_scaler; NEP_EINVAL if
+ * the file cannot be read or is inconsistent.  Prediction is then nep_load_structures (labels NULL) + nep_build_neighbors +
+ * nep_forward.  nep_get_model returns the hyper-parameters of a context (any pointer may be NULL): rc2 = {rc_R, rc_A},
+ * n_max2, basis2 = {radial, angular}, l_max3 = {l_max_3b, l_max_4b, l_max_5b}. */
+int nep_save_model(nep_ctx* ctx, const char* path);
+int nep_create_from_model_file(nep_ctx** out, const char* path, nep_alloc_fn alloc, nep_free_fn free_, void* alloc_user,
+                               void* cuda_stream);
+int nep_get_model(const nep_ctx* ctx, int* n_species, double* rc2, int* n_max2, int* basis2, int* l_max3, int* neurons);
 
 /* Releases every device buffer through free_ and the context itself.  NULL is a no-op. */
 int nep_destroy(nep_ctx* ctx);

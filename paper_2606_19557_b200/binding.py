@@ -28,6 +28,9 @@ SIGNATURES = {
     "nep_version": (C.c_char_p, []),
     "nep_create": (C.c_int, [C.POINTER(_P), C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                              C.c_int, C.c_int, C.c_int, ALLOC_FN, FREE_FN, _P, _P]),
+    "nep_save_model": (C.c_int, [_P, C.c_char_p]),
+    "nep_create_from_model_file": (C.c_int, [C.POINTER(_P), C.c_char_p, ALLOC_FN, FREE_FN, _P, _P]),
+    "nep_get_model": (C.c_int, [_P, C.POINTER(C.c_int), _P, _P, _P, _P, C.POINTER(C.c_int)]),
     "nep_destroy": (C.c_int, [_P]),
     "nep_last_error": (C.c_char_p, [_P]),
     "nep_num_descriptors": (C.c_int, [_P]),
@@ -103,8 +106,9 @@ def _ptr(a: Optional[np.ndarray]):
 class Nep:
     """One context = one CUDA device + one stream (include/nep.h).  Method names are the C calls without `nep_`."""
 
-    def __init__(self, n_species: int, rc_R: float, rc_A: float, n_max_R: int, n_max_A: int, basis_R: int, basis_A: int,
-                 l_max_3b: int = 4, l_max_4b: int = 2, l_max_5b: int = 1, neurons: int = 30, stream=None, guard_bytes: int = 0):
+    def __init__(self, n_species: int = 0, rc_R: float = 0.0, rc_A: float = 0.0, n_max_R: int = 0, n_max_A: int = 0, basis_R: int = 0,
+                 basis_A: int = 0, l_max_3b: int = 4, l_max_4b: int = 2, l_max_5b: int = 1, neurons: int = 30, stream=None,
+                 guard_bytes: int = 0, model_file: Optional[str] = None):
         import torch
         self._L = load_library()
         self._h = C.c_void_p(None)
@@ -150,8 +154,12 @@ class Nep:
         self._alloc_cb = ALLOC_FN(_alloc)
         self._free_cb = FREE_FN(_free)
         h = C.c_void_p(None)
-        rc = self._L.nep_create(C.byref(h), n_species, rc_R, rc_A, n_max_R, n_max_A, basis_R, basis_A, l_max_3b, l_max_4b,
-                                l_max_5b, neurons, self._alloc_cb, self._free_cb, None, C.c_void_p(stream.cuda_stream))
+        if model_file is not None:
+            rc = self._L.nep_create_from_model_file(C.byref(h), os.fsencode(model_file), self._alloc_cb, self._free_cb, None,
+                                                    C.c_void_p(stream.cuda_stream))
+        else:
+            rc = self._L.nep_create(C.byref(h), n_species, rc_R, rc_A, n_max_R, n_max_A, basis_R, basis_A, l_max_3b, l_max_4b,
+                                    l_max_5b, neurons, self._alloc_cb, self._free_cb, None, C.c_void_p(stream.cuda_stream))
         if rc != NEP_OK:
             raise NepError(rc, (self._L.nep_last_error(None) or b"").decode())
         self._h = h
@@ -175,6 +183,29 @@ class Nep:
         if bad:
             raise RuntimeError(f"guard bands overwritten next to {len(bad)} device buffers: {bad[:4]}")
         return len(getattr(self, "_guarded", {}))
+
+    @classmethod
+    def from_model_file(cls, path: str, **kw) -> "Nep":
+        """nep_create_from_model_file: hyper-parameters, scaler and parameters from a file written by save_model."""
+        return cls(model_file=path, **kw)
+
+    def save_model(self, path: str):
+        self._ck(self._L.nep_save_model(self._h, os.fsencode(path)))
+
+    def get_model(self) -> dict:
+        """Hyper-parameters of the context in the vocabulary of Table I."""
+        T, H = C.c_int(0), C.c_int(0)
+        rc = np.zeros(2, np.float64); nm = np.zeros(2, np.int32); bs = np.zeros(2, np.int32); lm = np.zeros(3, np.int32)
+        self._ck(self._L.nep_get_model(self._h, C.byref(T), _ptr(rc), _ptr(nm), _ptr(bs), _ptr(lm), C.byref(H)))
+        return dict(n_species=T.value, rc_R=float(rc[0]), rc_A=float(rc[1]), n_max_R=int(nm[0]), n_max_A=int(nm[1]), basis_R=int(bs[0]),
+                    basis_A=int(bs[1]), l_max_3b=int(lm[0]), l_max_4b=int(lm[1]), l_max_5b=int(lm[2]), neurons=H.value)
+
+    def predict(self, st):
+        """Prediction-only path: structures without labels in, (E [S], F [N,3], W [S,9]) out.  The calls are
+        nep_load_structures (labels NULL) + nep_build_neighbors + nep_forward; parameters and scaler stay as they are."""
+        self.load_structure_set(st)
+        self.build_neighbors()
+        return self.forward()
 
     @classmethod
     def from_model(cls, model, **kw) -> "Nep":

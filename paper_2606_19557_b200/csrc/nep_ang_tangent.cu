@@ -105,9 +105,9 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
             for (int l = 0; l < NL; ++l) S[l] = STAGED ? Ss[(n * NL + l) * WARP] : Sp[o + l * WARP];
             if (STAGED) {
 #pragma unroll
-                for (int sl = 0; sl < 4; ++sl) cf[sl] = Fs[(sl * m.nA + n0 + n) * WARP];
-                cf[4] = m.has4 ? Fs[(4 * m.nA + n0 + n) * WARP] : 0.0f;
-                cf[5] = m.has5 ? Fs[((4 + m.has4) * m.nA + n0 + n) * WARP] : 0.0f;
+                for (int sl = 0; sl < 4; ++sl) cf[sl] = sl < m.l3 ? Fs[(sl * m.nA + n0 + n) * WARP] : 0.0f;
+                cf[4] = m.has4 ? Fs[(m.l3 * m.nA + n0 + n) * WARP] : 0.0f;
+                cf[5] = m.has5 ? Fs[((m.l3 + m.has4) * m.nA + n0 + n) * WARP] : 0.0f;
             } else {
                 load_inv_coef(m, Fpp, n0 + n, cf);
             }

@@ -1,6 +1,7 @@
 // nep_api.cu -- C ABI entry points of libnep_b200 (include/nep.h): argument checks, state machine,
 // host<->device marshalling.  All arithmetic of the step lives in the kernels of the other .cu files.
 #include <math.h>
+#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 
@@ -127,7 +128,7 @@ int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max
     if (!(rc_A > 0.0) || !(rc_A <= rc_R) || !std::isfinite(rc_R)) return fail(nullptr, NEP_EINVAL, "need 0 < rc_A <= rc_R");
     if (n_max_R < 0 || n_max_A < 0 || n_max_R > 19 || n_max_A > 19) return fail(nullptr, NEP_EINVAL, "n_max must be in 0..19");
     if (basis_R < 1 || basis_A < 1 || basis_R > 16 || basis_A > 16) return fail(nullptr, NEP_EINVAL, "basis_size must be in 1..16");
-    if (l_max_3b != 4) return fail(nullptr, NEP_EINVAL, "l_max_3b must be 4");
+    if (l_max_3b < 1 || l_max_3b > 4) return fail(nullptr, NEP_EINVAL, "l_max_3b must be in 1..4");
     if (!(l_max_4b == 0 || l_max_4b == 2)) return fail(nullptr, NEP_EINVAL, "l_max_4b must be 0 or 2");
     if (!(l_max_5b == 0 || l_max_5b == 1)) return fail(nullptr, NEP_EINVAL, "l_max_5b must be 0 or 1");
     if (neurons < 1 || neurons > 512) return fail(nullptr, NEP_EINVAL, "neurons must be in 1..512");
@@ -144,7 +145,7 @@ int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max
     c->alloc = alloc; c->free_ = free_; c->user = alloc_user; c->stream = (cudaStream_t)cuda_stream;
     ModelDev& m = c->m;
     m.T = n_species; m.nR = n_max_R + 1; m.nA = n_max_A + 1; m.KR = basis_R + 1; m.KA = basis_A + 1; m.KRP = (m.KR + 3) & ~3;
-    m.H = neurons; m.has4 = l_max_4b > 0; m.has5 = l_max_5b > 0; m.nang = 4 + m.has4 + m.has5;
+    m.H = neurons; m.has4 = l_max_4b > 0; m.has5 = l_max_5b > 0; m.l3 = l_max_3b; m.nang = m.l3 + m.has4 + m.has5;
     m.D = m.nR + m.nA * m.nang; m.DP = (m.D + 7) & ~7; m.HP = (m.H + 7) & ~7;
     m.rcR = (float)rc_R; m.rcA = (float)rc_A; m.rcinvR = (float)(1.0 / rc_R); m.rcinvA = (float)(1.0 / rc_A);
     m.per_type = (m.D + 2) * m.H; m.o_b1 = m.per_type * m.T; m.o_cR = m.o_b1 + 1; m.o_cA = m.o_cR + m.T * m.T * m.nR * m.KR;
@@ -382,6 +383,75 @@ int nep_get_grad(nep_ctx* c, float* g)
     if (!g) return fail(c, NEP_EINVAL, "g is NULL");
     if (!c->grad_valid) return fail(c, NEP_ESTATE, "no gradient: call nep_loss_grad (or nep_set_grad) first");
     return d2h(c, g, c->g, 4 * (size_t)c->m.npar);
+}
+// ---- a model as a file: hyper-parameters of Table I, the scaler of Eq. 2 and theta (layout DESIGN C0) ----
+static const char* const MODEL_MAGIC = "nep_b200_model";
+int nep_save_model(nep_ctx* c, const char* path)
+{
+    CHECK_CTX(c);
+    if (!path) return fail(c, NEP_EINVAL, "path is NULL");
+    if (!c->have_params || !c->have_scaler) return fail(c, NEP_ESTATE, "nep_save_model needs parameters and a scaler");
+    std::vector<float> th(c->m.npar);
+    std::vector<double> sc(c->m.D);
+    int rc = nep_get_params(c, th.data());
+    if (rc) return rc;
+    if ((rc = nep_get_scaler(c, sc.data()))) return rc;
+    FILE* f = fopen(path, "w");
+    if (!f) return fail(c, NEP_EINVAL, std::string("cannot open ") + path + " for writing");
+    fprintf(f, "%s 1\n", MODEL_MAGIC);
+    fprintf(f, "n_species %d\ncutoff %.17g %.17g\nn_max %d %d\nbasis_size %d %d\nl_max %d %d %d\nneuron %d\n", c->m.T, c->rcR, c->rcA,
+            c->n_max_R, c->n_max_A, c->basis_R, c->basis_A, c->l3, c->l4, c->l5, c->m.H);
+    fprintf(f, "scaler %d\n", c->m.D);
+    for (int i = 0; i < c->m.D; ++i) fprintf(f, "%.9g\n", sc[i]);          // the scaler is held in fp32 on the device
+    fprintf(f, "theta %d\n", c->m.npar);
+    for (int i = 0; i < c->m.npar; ++i) fprintf(f, "%.9g\n", th[i]);       // 9 significant digits round-trip an fp32 value
+    const bool ok = !ferror(f);
+    if (fclose(f) != 0 || !ok) return fail(c, NEP_EINVAL, std::string("write error on ") + path);
+    return NEP_OK;
+}
+int nep_create_from_model_file(nep_ctx** out, const char* path, nep_alloc_fn alloc, nep_free_fn free_, void* alloc_user, void* cuda_stream)
+{
+    if (!out) return fail(nullptr, NEP_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!path) return fail(nullptr, NEP_EINVAL, "path is NULL");
+    FILE* f = fopen(path, "r");
+    if (!f) return fail(nullptr, NEP_EINVAL, std::string("cannot open ") + path);
+    char magic[32] = {0};
+    int ver = 0, T = 0, nmR = 0, nmA = 0, bR = 0, bA = 0, l3 = 0, l4 = 0, l5 = 0, H = 0, D = 0, npar = 0;
+    double rcR = 0, rcA = 0;
+    bool ok = fscanf(f, "%31s %d", magic, &ver) == 2 && std::string(magic) == MODEL_MAGIC && ver == 1;
+    ok = ok && fscanf(f, " n_species %d cutoff %lf %lf n_max %d %d basis_size %d %d l_max %d %d %d neuron %d scaler %d", &T, &rcR, &rcA, &nmR,
+                      &nmA, &bR, &bA, &l3, &l4, &l5, &H, &D) == 12;
+    if (!ok) { fclose(f); return fail(nullptr, NEP_EINVAL, std::string(path) + " is not a nep_b200 model file (version 1)"); }
+    nep_ctx* c = nullptr;
+    int rc = nep_create(&c, T, rcR, rcA, nmR, nmA, bR, bA, l3, l4, l5, H, alloc, free_, alloc_user, cuda_stream);
+    if (rc) { fclose(f); return rc; }
+    std::vector<double> sc(c->m.D);
+    std::vector<float> th(c->m.npar);
+    ok = D == c->m.D;
+    for (int i = 0; ok && i < D; ++i) ok = fscanf(f, "%lf", &sc[i]) == 1;
+    ok = ok && fscanf(f, " theta %d", &npar) == 1 && npar == c->m.npar;
+    for (int i = 0; ok && i < npar; ++i) ok = fscanf(f, "%f", &th[i]) == 1;
+    fclose(f);
+    if (!ok) { nep_destroy(c); return fail(nullptr, NEP_EINVAL, std::string(path) + ": sizes or values do not match the header"); }
+    if ((rc = nep_set_params(c, th.data())) || (rc = nep_set_scaler(c, sc.data()))) {
+        g_create_error = c->err;
+        nep_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return NEP_OK;
+}
+int nep_get_model(const nep_ctx* c, int* n_species, double* rc2, int* n_max2, int* basis2, int* l_max3, int* neurons)
+{
+    if (!c) return NEP_EINVAL;
+    if (n_species) *n_species = c->m.T;
+    if (rc2) { rc2[0] = c->rcR; rc2[1] = c->rcA; }
+    if (n_max2) { n_max2[0] = c->n_max_R; n_max2[1] = c->n_max_A; }
+    if (basis2) { basis2[0] = c->basis_R; basis2[1] = c->basis_A; }
+    if (l_max3) { l_max3[0] = c->l3; l_max3[1] = c->l4; l_max3[2] = c->l5; }
+    if (neurons) *neurons = c->m.H;
+    return NEP_OK;
 }
 int nep_set_grad(nep_ctx* c, const float* g)
 {

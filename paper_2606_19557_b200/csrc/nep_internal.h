@@ -22,7 +22,7 @@ constexpr int MAX_NCH = 5;   // angular channels held in registers by one thread
 
 // Everything a kernel needs to know about the model (passed by value).
 struct ModelDev {
-    int T, nR, nA, KR, KA, KRP, H, HP, D, DP, nang, has4, has5;   // HP, DP: H, D padded to multiples of 8; KRP: KR to 4
+    int T, nR, nA, KR, KA, KRP, H, HP, D, DP, nang, l3, has4, has5;   // HP, DP: H, D padded to multiples of 8; KRP: KR to 4; l3: 3-body orders l = 1..l3
     float rcR, rcA, rcinvR, rcinvA;
     // offsets into theta
     int per_type;          // (D + 2) * H

@@ -338,21 +338,22 @@ __device__ __forceinline__ void radial_gn(float r, float rcinv, const float* __r
 // descriptor rows of the angular invariants of channel n: slots 0..3 -> l = 1..4, slot 4 -> 4-body, slot 5 -> 5-body
 __device__ __forceinline__ int ang_row(const ModelDev& m, int slot, int n)
 {
-    const int a = slot < 4 ? slot : (slot == 4 ? 4 : 4 + m.has4);
+    const int a = slot < 4 ? slot : (slot == 4 ? m.l3 : m.l3 + m.has4);   // callers use a 3-body slot only if slot < l3
     return m.nR + a * m.nA + n;
 }
 // c[slot] = arr[row(slot, n)] for the invariants present, 0 otherwise  (arr: slice-blocked [D] rows, pointer at row 0)
 __device__ __forceinline__ void load_inv_coef(const ModelDev& m, const float* __restrict__ arr, int n, float* c)
 {
 #pragma unroll
-    for (int s = 0; s < 4; ++s) c[s] = arr[(size_t)ang_row(m, s, n) * WARP];
+    for (int s = 0; s < 4; ++s) c[s] = s < m.l3 ? arr[(size_t)ang_row(m, s, n) * WARP] : 0.0f;
     c[4] = m.has4 ? arr[(size_t)ang_row(m, 4, n) * WARP] : 0.0f;
     c[5] = m.has5 ? arr[(size_t)ang_row(m, 5, n) * WARP] : 0.0f;
 }
 __device__ __forceinline__ void store_inv(const ModelDev& m, float* __restrict__ arr, int n, const float* q)
 {
 #pragma unroll
-    for (int s = 0; s < 4; ++s) arr[(size_t)ang_row(m, s, n) * WARP] = q[s];
+    for (int s = 0; s < 4; ++s)
+        if (s < m.l3) arr[(size_t)ang_row(m, s, n) * WARP] = q[s];
     if (m.has4) arr[(size_t)ang_row(m, 4, n) * WARP] = q[4];
     if (m.has5) arr[(size_t)ang_row(m, 5, n) * WARP] = q[5];
 }
@@ -387,7 +388,7 @@ __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n
 #pragma unroll
         for (int l = 0; l < NL; ++l) S[n][l] = __ldg(sp + l * WARP);
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Fpp + (size_t)ang_row(m, s, nn) * WARP);
+        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Fpp + (size_t)ang_row(m, s < m.l3 ? s : 0, nn) * WARP);
         coef[n][4] = __ldg(Fpp + (size_t)ang_row(m, m.has4 ? 4 : 0, nn) * WARP);
         coef[n][5] = __ldg(Fpp + (size_t)ang_row(m, m.has5 ? 5 : 0, nn) * WARP);
     }
@@ -395,7 +396,7 @@ __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n
     for (int n = 0; n < NCH; ++n) {
         const bool ok = n0 + n < m.nA && L.ti >= 0;
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[n][s] = ok ? coef[n][s] : 0.0f;
+        for (int s = 0; s < 4; ++s) coef[n][s] = (ok && s < m.l3) ? coef[n][s] : 0.0f;
         coef[n][4] = (ok && m.has4) ? coef[n][4] : 0.0f;
         coef[n][5] = (ok && m.has5) ? coef[n][5] : 0.0f;
         inv_adjoint(S[n], coef[n], EdS[n]);
@@ -420,7 +421,7 @@ __device__ __forceinline__ void load_Sbar(const StepArgs& a, const Lane& L, int 
 #pragma unroll
         for (int l = 0; l < NL; ++l) { S[n][l] = __ldg(sp + l * WARP); X[n][l] = __ldg(hp + l * WARP); }
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Qbp + (size_t)ang_row(m, s, nn) * WARP);
+        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Qbp + (size_t)ang_row(m, s < m.l3 ? s : 0, nn) * WARP);
         coef[n][4] = __ldg(Qbp + (size_t)ang_row(m, m.has4 ? 4 : 0, nn) * WARP);
         coef[n][5] = __ldg(Qbp + (size_t)ang_row(m, m.has5 ? 5 : 0, nn) * WARP);
     }
@@ -428,7 +429,7 @@ __device__ __forceinline__ void load_Sbar(const StepArgs& a, const Lane& L, int 
     for (int n = 0; n < NCH; ++n) {
         const bool ok = n0 + n < m.nA && L.ti >= 0;
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[n][s] = ok ? coef[n][s] : 0.0f;
+        for (int s = 0; s < 4; ++s) coef[n][s] = (ok && s < m.l3) ? coef[n][s] : 0.0f;
         coef[n][4] = (ok && m.has4) ? coef[n][4] : 0.0f;
         coef[n][5] = (ok && m.has5) ? coef[n][5] : 0.0f;
         float t[NL];
@@ -451,9 +452,9 @@ __device__ __forceinline__ void load_EdS_staged(const ModelDev& m, int ti, int n
 #pragma unroll
         for (int l = 0; l < NL; ++l) S[l] = ok ? Ss[(n * NL + l) * WARP] : 0.0f;
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[s] = ok ? Fs[(s * m.nA + nn) * WARP] : 0.0f;
-        coef[4] = (ok && m.has4) ? Fs[(4 * m.nA + nn) * WARP] : 0.0f;
-        coef[5] = (ok && m.has5) ? Fs[((4 + m.has4) * m.nA + nn) * WARP] : 0.0f;
+        for (int s = 0; s < 4; ++s) coef[s] = (ok && s < m.l3) ? Fs[(s * m.nA + nn) * WARP] : 0.0f;
+        coef[4] = (ok && m.has4) ? Fs[(m.l3 * m.nA + nn) * WARP] : 0.0f;
+        coef[5] = (ok && m.has5) ? Fs[((m.l3 + m.has4) * m.nA + nn) * WARP] : 0.0f;
         inv_adjoint(S, coef, EdS[n]);
     }
 }

@@ -49,8 +49,11 @@ def test_create_without_gpu_fails_loudly_or_validates(built):
     assert rc == binding.NEP_EINVAL and b"n_species" in L.nep_last_error(None)
     rc = L.nep_create(ctypes.byref(h), 1, 4.0, 5.0, 4, 4, 8, 8, 4, 2, 1, 30, null_a, null_f, None, None)
     assert rc == binding.NEP_EINVAL
-    rc = L.nep_create(ctypes.byref(h), 1, 5.0, 4.0, 4, 4, 8, 8, 3, 2, 1, 30, null_a, null_f, None, None)
-    assert rc == binding.NEP_EINVAL
+    for l3, l4, l5 in ((0, 2, 1), (5, 2, 1), (4, 1, 1), (4, 2, 2)):          # l_max_3b in 1..4, l_max_4b in {0,2}, l_max_5b in {0,1}
+        rc = L.nep_create(ctypes.byref(h), 1, 5.0, 4.0, 4, 4, 8, 8, l3, l4, l5, 30, null_a, null_f, None, None)
+        assert rc == binding.NEP_EINVAL and b"l_max" in L.nep_last_error(None)
+    rc = L.nep_create_from_model_file(ctypes.byref(h), b"/nonexistent/model.txt", null_a, null_f, None, None)
+    assert rc == binding.NEP_EINVAL and b"cannot open" in L.nep_last_error(None)
     import torch
     if not torch.cuda.is_available():
         rc = L.nep_create(ctypes.byref(h), 1, 5.0, 4.0, 4, 4, 8, 8, 4, 2, 1, 30, null_a, null_f, None, None)

@@ -21,6 +21,11 @@ def _cases():
         "tiny_3body_only": lambda: wl.tiny_workload(3, model=wl.ModelSpec(2, 3.2, 2.6, 2, 0, 3, 1, 4, 0, 0, 5)),
         "tiny_4body_only": lambda: wl.tiny_workload(4, model=wl.ModelSpec(2, 3.2, 3.2, 0, 2, 1, 3, 4, 2, 0, 3)),
         "tiny_5body_only": lambda: wl.tiny_workload(5, model=wl.ModelSpec(2, 3.0, 2.0, 1, 1, 2, 2, 4, 0, 1, 9)),
+        # other three-body orders: l_max_3b = 1, 2, 3 with and without the 4-/5-body terms
+        "tiny_l3_1_5body": lambda: wl.tiny_workload(8, model=wl.ModelSpec(2, 3.2, 2.6, 2, 2, 3, 3, 1, 0, 1, 5)),
+        "tiny_l3_2_4body": lambda: wl.tiny_workload(9, model=wl.ModelSpec(2, 3.2, 2.8, 1, 3, 2, 4, 2, 2, 0, 6)),
+        "tiny_l3_3_full": lambda: wl.tiny_workload(10, n_species=3, sizes=(33, 2, 40), box=(7.5, 3.1, 8.0),
+                                                   model=wl.ModelSpec(3, 3.2, 2.6, 2, 5, 3, 4, 3, 2, 1, 7)),
         "cfg1a": lambda: wl.make_config(1),
         "cfg1b": lambda: wl.make_config(1, n_struct=2, variant="1b"),
         "cfg2": lambda: wl.make_config(2, n_struct=6),
