@@ -314,6 +314,9 @@ def run_ours(args):
         dist.barrier()
     torch.cuda.synchronize()
     clocks = ClockSampler(local) if rank == 0 else None
+    for i in range(3):                 # starting the sampler leaves the GPU idle for a moment: more untimed steps, then the timed region
+        set_b(i); one_step(nep, lam, graph=True)
+    torch.cuda.synchronize()
     l0 = nep.launch_count()
     t0 = time.time()
     for i in range(K):

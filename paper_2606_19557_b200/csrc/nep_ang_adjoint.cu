@@ -2,8 +2,9 @@
 //   g_cA[ti][tj][n][k] += [sum_L Sb_nL b_L + sum_L EdS_nL (grad b_L . d~)] f_k + [sum_L EdS_nL b_L] (r^.d~) f_k'
 // The two terms need different per-atom tensors in registers (Sb = J^T Qb + HS, and EdS = dE_i/dS), so they are two PASSES over
 // the pair records.  A thread accumulates acc[n][k] over its pairs.
-// One species (k_ang_adjoint): a block runs both passes and shuffle-reduces the accumulators; the per-atom rows of the second pass
-// are requested into shared memory before the first pass starts (rows_request), those of the first pass are loaded branch free.
+// One species (k_ang_adjoint): a block runs both passes and shuffle-reduces the accumulators; the per-atom rows come through the
+// warp's shared-memory area (rows_request): those of the first pass are requested at kernel entry, those of the second pass as soon
+// as the first pass has formed its tensor, so that they arrive while the first pass runs.
 // Several species (k_ang_adjoint_ms): one warp per block and pass, snapshot table (below).
 #include <algorithm>
 
@@ -24,12 +25,10 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
     const int wib = threadIdx.x >> 5;
     float* area = tab_all + (size_t)nwarp * NKP + (size_t)wib * staged_warp_floats(m, NCH);
     uint64_t* mbar = reinterpret_cast<uint64_t*>(tab_all + (size_t)nwarp * NKP + (size_t)nwarp * staged_warp_floats(m, NCH)) + wib;
-    if (STAGED) {   // rows of pass 1, on their way while pass 0 runs
-        const size_t w = (size_t)blockIdx.x * nwarp + wib;
-        if (w < (size_t)a.b.nbs)
-            rows_request(mbar, area, a.b.S + (w * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
-                         area + NCH * NL * WARP, a.b.Fp + (w * m.D + m.nR) * WARP, m.D - m.nR);
-    }
+    const size_t wg = (size_t)blockIdx.x * nwarp + wib;
+    if (STAGED && wg < (size_t)a.b.nbs)   // pass 0: tangent moments of the chunk and the angular rows of Qb
+        rows_request(mbar, area, a.b.Sd + (wg * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
+                     area + NCH * NL * WARP, a.b.Qb + (wg * m.D + m.nR) * WARP, m.D - m.nR);
     Lane L;
     const bool inb = lane_init(a, L);
     constexpr int KH = (K + 1) / 2;
@@ -48,7 +47,14 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             // ---- pass 0: Sb ----
             {
                 float X[NCH][NL];
-                load_Sbar<NCH>(a, L, n0, X);
+                if (STAGED) {
+                    load_Sbar_staged<NCH>(a, L, n0, area + L.lane, area + NCH * NL * WARP + L.lane, mbar, X);
+                    // the area is free again: rows of pass 1 (moments, angular rows of Fp), on their way while pass 0 runs
+                    rows_request(mbar, area, a.b.S + (wg * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
+                                 area + NCH * NL * WARP, a.b.Fp + (wg * m.D + m.nR) * WARP, m.D - m.nR, true);
+                } else {
+                    load_Sbar<NCH>(a, L, n0, X);
+                }
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) pack24(X[n], X2[n]);
             }
@@ -91,7 +97,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             {
                 float X[NCH][NL];
                 if (STAGED) {
-                    rows_wait(mbar);
+                    rows_wait(mbar, 1);
                     load_EdS_staged<NCH>(m, L.ti, n0, area + L.lane, area + NCH * NL * WARP + L.lane, X);
                 } else {
                     load_EdS<NCH>(a, L, n0, X);

@@ -1,14 +1,11 @@
 // nep_ang_tangent.cu -- S7 (angular part), the tangent sweep of the second-order path (DESIGN C10):
 //   Sd_nL = sum_j [g_n'(r) (r^ . d~) b_L + g_n(r) (grad_d b_L . d~)],   d~_ij = u_i - u_j - G_s^T d_ij,
 //   qd_ang = J_q(S) Sd.
-// The epilogue also forms the second-derivative term of the adjoint sweep's per-atom tensor (DESIGN C12),
-//   HS_nL = sum_nu Fp_nu (H_{q_nu} Sd)_nL,
-// while S and Sd are on chip, and stores it in place of Sd (nothing else reads Sd).
 #include "nep_kernels.cuh"
 
 namespace nep {
 
-// STAGED: the rows the epilogue reads (moments of the chunk, angular rows of Fp) are requested into shared memory before the sweep.
+// STAGED: the rows the epilogue reads (moments of the chunk) are requested into shared memory before the sweep.
 template <int NCH, int K, bool STAGED>
 __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
 {
@@ -20,13 +17,11 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
     const int n0 = blockIdx.y * NCH;
     const int wib = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     float* area0 = cs + ((m.T * m.T * CST + 3) & ~3);
-    float* area = area0 + (size_t)wib * staged_warp_floats(m, NCH);
-    uint64_t* mbar = reinterpret_cast<uint64_t*>(area0 + (size_t)nwarp * staged_warp_floats(m, NCH)) + wib;
+    float* area = area0 + (size_t)wib * (NCH * NL * WARP);
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(area0 + (size_t)nwarp * (NCH * NL * WARP)) + wib;
     if (STAGED) {
         const size_t w = (size_t)blockIdx.x * nwarp + wib;
-        if (w < (size_t)a.b.nbs)
-            rows_request(mbar, area, a.b.S + (w * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
-                         area + NCH * NL * WARP, a.b.Fp + (w * m.D + m.nR) * WARP, m.D - m.nR);
+        if (w < (size_t)a.b.nbs) rows_request(mbar, area, a.b.S + (w * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH), nullptr, nullptr, 0);
     }
     Lane L;
     const bool inb = lane_init(a, L);
@@ -90,36 +85,21 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
     for (int n = 0; n < NCH; ++n) unpack24(Sd2[n], Sd[n]);
     if (STAGED) rows_wait(mbar);
     const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
-    const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
     const float* Ss = area + L.lane;
-    const float* Fs = area + NCH * NL * WARP + L.lane;
-    float* HSp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
+    float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
     float* qdp = sb_ptr(a.b.qd, L.w, m.D, L.lane);
-    const bool live = L.ti >= 0;
 #pragma unroll
     for (int n = 0; n < NCH; ++n) {
         if (n0 + n < m.nA) {
-            float S[NL], qd[6], cf[6], HS[NL];
+            float S[NL], qd[6];
             const size_t o = (size_t)(n0 + n) * NL * WARP;
 #pragma unroll
-            for (int l = 0; l < NL; ++l) S[l] = STAGED ? Ss[(n * NL + l) * WARP] : Sp[o + l * WARP];
-            if (STAGED) {
-#pragma unroll
-                for (int sl = 0; sl < 4; ++sl) cf[sl] = sl < m.l3 ? Fs[(sl * m.nA + n0 + n) * WARP] : 0.0f;
-                cf[4] = m.has4 ? Fs[(m.l3 * m.nA + n0 + n) * WARP] : 0.0f;
-                cf[5] = m.has5 ? Fs[((m.l3 + m.has4) * m.nA + n0 + n) * WARP] : 0.0f;
-            } else {
-                load_inv_coef(m, Fpp, n0 + n, cf);
+            for (int l = 0; l < NL; ++l) {
+                S[l] = STAGED ? Ss[(n * NL + l) * WARP] : Sp[o + l * WARP];
+                Sdp[o + l * WARP] = Sd[n][l];
             }
-#pragma unroll
-            for (int sl = 0; sl < 6; ++sl) cf[sl] = live ? cf[sl] : 0.0f;   // padding lanes: Fp is not defined there
             inv_tangent(S, Sd[n], qd);
             store_inv(m, qdp, n0 + n, qd);
-#pragma unroll
-            for (int l = 0; l < NL; ++l) HS[l] = 0.0f;
-            inv_hessian_action(S, Sd[n], cf, HS);
-#pragma unroll
-            for (int l = 0; l < NL; ++l) HSp[o + l * WARP] = HS[l];
         }
     }
 }
@@ -131,7 +111,7 @@ int launch_ang_tangent(nep_ctx* c, const StepArgs& a)
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
         const size_t base = SWEEP2_SMEM_BYTES + ((cA_chunk_bytes<NCH, K>(m) + 15) & ~(size_t)15);
-        const size_t smem = base + 4 * (PAIR_TB / WARP) * staged_warp_floats(m, NCH) + STAGED_BAR_BYTES;
+        const size_t smem = base + 4 * (size_t)(PAIR_TB / WARP) * (NCH * NL * WARP) + STAGED_BAR_BYTES;
         if (2 * smem + 2048 <= (size_t)c->max_smem_sm) {      // two blocks per SM (the register limit) keep fitting
             auto kern = k_ang_tangent<NCH, K, true>;
             if (smem > 48 * 1024) NEP_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -250,11 +250,15 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  :: "r"(umma::smem_u32(dst)), "l"(src), "r"(bytes), "r"(umma::smem_u32(mbar)) : "memory");
 }
 // whole warp calls; two blocks of rows (either may be empty).  rows_wait afterwards, by every lane, before the first read.
-__device__ __forceinline__ void rows_request(uint64_t* mbar, float* dst0, const float* src0, int rows0, float* dst1, const float* src1, int rows1)
+// A warp may use its area a second time (again = true, after every lane has finished reading the first contents): the mbarrier then
+// completes its next phase, awaited with parity 1.
+__device__ __forceinline__ void rows_request(uint64_t* mbar, float* dst0, const float* src0, int rows0, float* dst1, const float* src1, int rows1,
+                                             bool again = false)
 {
+    __syncwarp();
     if ((threadIdx.x & 31) == 0) {
-        umma::mbar_init(mbar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (!again) umma::mbar_init(mbar, 1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // barrier initialised / area read: visible to the async proxy
         const uint32_t b0 = (uint32_t)rows0 * (4 * WARP), b1 = (uint32_t)rows1 * (4 * WARP);
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(umma::smem_u32(mbar)), "r"(b0 + b1) : "memory");
         if (b0) bulk_g2s(dst0, src0, b0, mbar);
@@ -262,7 +266,7 @@ __device__ __forceinline__ void rows_request(uint64_t* mbar, float* dst0, const 
     }
     __syncwarp();
 }
-__device__ __forceinline__ void rows_wait(uint64_t* mbar) { umma::mbar_wait(mbar, 0); }
+__device__ __forceinline__ void rows_wait(uint64_t* mbar, uint32_t parity = 0) { umma::mbar_wait(mbar, parity); }
 
 struct SweepA { const float4* rec; int width, cnt; };
 __device__ __forceinline__ SweepA sweep_init(const int64_t* __restrict__ recoff, const float4* __restrict__ recs,
@@ -403,39 +407,85 @@ __device__ __forceinline__ void load_EdS(const StepArgs& a, const Lane& L, int n
     }
 }
 
-// Sb_nL = sum_a Qb[(a, n)] dq_a/dS_nL + HS_nL: the per-atom tensor of the first pass of the adjoint sweep (DESIGN C12); HS is the
-// second-derivative term that the tangent sweep left in b.Sd.  Branch free like load_EdS.
+// Sb_nL = sum_a Qb[(a, n)] dq_a/dS_nL + sum_a Fp[(a, n)] (H_{q_a} Sd)_nL: the per-atom tensor of the first pass of the adjoint sweep
+// (DESIGN C12).  Branch free like load_EdS.
 template <int NCH>
 __device__ __forceinline__ void load_Sbar(const StepArgs& a, const Lane& L, int n0, float (*X)[NL])
 {
     const ModelDev& m = a.m;
     const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
-    const float* Hp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
+    const float* Sdp = sb_ptr(a.b.Sd, L.w, m.nA * NL, L.lane);
     const float* Qbp = sb_ptr(a.b.Qb, L.w, m.D, L.lane);
-    float S[NCH][NL], coef[NCH][6];
+    const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
+#pragma unroll
+    for (int n = 0; n < NCH; ++n) {
+        const bool ok = n0 + n < m.nA && L.ti >= 0;
+        const int nn = n0 + n < m.nA ? n0 + n : m.nA - 1;
+        const float* sp = Sp + (size_t)nn * NL * WARP;
+        const float* dp = Sdp + (size_t)nn * NL * WARP;
+        float S[NL], Sd[NL], cq[6], cf[6];
+#pragma unroll
+        for (int l = 0; l < NL; ++l) { S[l] = __ldg(sp + l * WARP); Sd[l] = __ldg(dp + l * WARP); }
+#pragma unroll
+        for (int s = 0; s < 6; ++s) {
+            const int slot = (s < 4 ? s < m.l3 : (s == 4 ? m.has4 : m.has5)) ? s : 0;
+            cq[s] = __ldg(Qbp + (size_t)ang_row(m, slot, nn) * WARP);
+            cf[s] = __ldg(Fpp + (size_t)ang_row(m, slot, nn) * WARP);
+        }
+#pragma unroll
+        for (int s = 0; s < 6; ++s) {
+            const bool on = ok && (s < 4 ? s < m.l3 : (s == 4 ? m.has4 : m.has5));
+            cq[s] = on ? cq[s] : 0.0f; cf[s] = on ? cf[s] : 0.0f;
+        }
+        inv_adjoint(S, cq, X[n]);
+        inv_hessian_action(S, Sd, cf, X[n]);
+        if (!ok)
+#pragma unroll
+            for (int l = 0; l < NL; ++l) X[n][l] = 0.0f;
+    }
+}
+
+// load_Sbar with Sd (chunk rows) and the angular rows of Qb staged in shared memory (Ds, Qs: this lane's column); S and the
+// coefficients from Fp come straight from global memory, all loads issued before the staged rows are awaited.
+template <int NCH>
+__device__ __forceinline__ void load_Sbar_staged(const StepArgs& a, const Lane& L, int n0, const float* Ds, const float* Qs, uint64_t* mbar,
+                                                 float (*X)[NL])
+{
+    const ModelDev& m = a.m;
+    const float* Sp = sb_ptr(a.b.S, L.w, m.nA * NL, L.lane);
+    const float* Fpp = sb_ptr(a.b.Fp, L.w, m.D, L.lane);
+    float cf[NCH][6];
 #pragma unroll
     for (int n = 0; n < NCH; ++n) {
         const int nn = n0 + n < m.nA ? n0 + n : m.nA - 1;
         const float* sp = Sp + (size_t)nn * NL * WARP;
-        const float* hp = Hp + (size_t)nn * NL * WARP;
 #pragma unroll
-        for (int l = 0; l < NL; ++l) { S[n][l] = __ldg(sp + l * WARP); X[n][l] = __ldg(hp + l * WARP); }
+        for (int l = 0; l < NL; ++l) X[n][l] = __ldg(sp + l * WARP);          // S for now
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[n][s] = __ldg(Qbp + (size_t)ang_row(m, s < m.l3 ? s : 0, nn) * WARP);
-        coef[n][4] = __ldg(Qbp + (size_t)ang_row(m, m.has4 ? 4 : 0, nn) * WARP);
-        coef[n][5] = __ldg(Qbp + (size_t)ang_row(m, m.has5 ? 5 : 0, nn) * WARP);
+        for (int s = 0; s < 6; ++s) {
+            const int slot = (s < 4 ? s < m.l3 : (s == 4 ? m.has4 : m.has5)) ? s : 0;
+            cf[n][s] = __ldg(Fpp + (size_t)ang_row(m, slot, nn) * WARP);
+        }
     }
+    rows_wait(mbar, 0);
 #pragma unroll
     for (int n = 0; n < NCH; ++n) {
         const bool ok = n0 + n < m.nA && L.ti >= 0;
+        const int nn = n0 + n < m.nA ? n0 + n : m.nA - 1;
+        float S[NL], Sd[NL], cq[6], out[NL];
 #pragma unroll
-        for (int s = 0; s < 4; ++s) coef[n][s] = (ok && s < m.l3) ? coef[n][s] : 0.0f;
-        coef[n][4] = (ok && m.has4) ? coef[n][4] : 0.0f;
-        coef[n][5] = (ok && m.has5) ? coef[n][5] : 0.0f;
-        float t[NL];
-        inv_adjoint(S[n], coef[n], t);
+        for (int l = 0; l < NL; ++l) { S[l] = X[n][l]; Sd[l] = ok ? Ds[(n * NL + l) * WARP] : 0.0f; }
 #pragma unroll
-        for (int l = 0; l < NL; ++l) X[n][l] = ok ? t[l] + X[n][l] : 0.0f;
+        for (int s = 0; s < 6; ++s) {
+            const bool on = ok && (s < 4 ? s < m.l3 : (s == 4 ? m.has4 : m.has5));
+            const int row = s < 4 ? s : (s == 4 ? m.l3 : m.l3 + m.has4);
+            cq[s] = on ? Qs[(row * m.nA + nn) * WARP] : 0.0f;
+            cf[n][s] = on ? cf[n][s] : 0.0f;
+        }
+        inv_adjoint(S, cq, out);
+        inv_hessian_action(S, Sd, cf[n], out);
+#pragma unroll
+        for (int l = 0; l < NL; ++l) X[n][l] = ok ? out[l] : 0.0f;
     }
 }
 
