@@ -309,6 +309,9 @@ def run_ours(args):
     # ---- timed region: K steps, CUDA events per step on the launching stream, L2 flushed between steps ----
     K = args.steps
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    # one event pair per step where something that is not part of the step sits between steps (the flush; the selection of the next
+    # batch, whose table upload belongs to the e2e number); one pair around all K steps where the same batch is stepped back to back
+    per_step = flush is not None or not single
     atoms = structs = 0
     if world > 1:
         dist.barrier()
@@ -325,10 +328,10 @@ def run_ours(args):
             flush.fill_(i & 0xFF)
         sz = nep.batch_shape()
         structs += sz[0]; atoms += sz[1]
-        if flush is not None or i == 0:
+        if per_step or i == 0:
             ev[i][0].record()
         one_step(nep, lam, graph=True)
-        if flush is not None or i == K - 1:
+        if per_step or i == K - 1:
             ev[i][1].record()
     torch.cuda.synchronize()
     t1 = time.time()
@@ -348,8 +351,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     prof = nep.profile_read()
     nep.profile_enable(False)
-    # flushed: the sum of the per-step event pairs (the flush is outside them); not flushed: one pair around the K steps
-    total_ms = float(sum(a.elapsed_time(b) for a, b in ev)) if flush is not None else float(ev[0][0].elapsed_time(ev[K - 1][1]))
+    total_ms = float(sum(a.elapsed_time(b) for a, b in ev)) if per_step else float(ev[0][0].elapsed_time(ev[K - 1][1]))
     if world > 1:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -372,6 +374,13 @@ def run_ours(args):
         set_b(i); one_step(nep, lam, graph=False)
     b.record(); torch.cuda.synchronize()
     ms_b2b_stream = a.elapsed_time(b) / K
+
+    # ---- prediction only: nep_forward alone (descriptors, network, E, F, virial), back to back ----
+    a.record()
+    for i in range(K):
+        set_b(i); nep.forward_device()
+    b.record(); torch.cuda.synchronize()
+    ms_predict = a.elapsed_time(b) / K
 
     # ---- sustained: seconds of back-to-back steps under the power cap, clocks and power sampled (the timed region above is short) ----
     sustained = None
@@ -467,8 +476,11 @@ def run_ours(args):
         "config": {"workload": workload_name(w, args), "structures_per_s": structs / (total_ms * 1e-3),
                    "atoms_per_step": atoms // K // world, "pairs_R_per_step": sizes["P_R_b"], "pairs_A_per_step": sizes["P_A_b"],
                    "l2": ("flushed between timed steps (256 MB write)" if flush is not None else
-                          f"inputs larger than L2: one step streams {step_bytes / 1e6:.0f} MB (algorithmic bytes) through a {L2_BYTES / 1e6:.0f} MB L2; steps timed back to back, no flush"),
+                          f"inputs larger than L2: one step streams {step_bytes / 1e6:.0f} MB (algorithmic bytes) through a {L2_BYTES / 1e6:.0f} MB L2; no flush"
+                          + ("; the K steps between one event pair" if single else "; one event pair per step (the next batch is selected between them)")),
                    "ms_per_step_back_to_back_no_flush": ms_b2b, "ms_per_step_back_to_back_three_calls": ms_b2b_stream,
+                   "predict_only": {"ms_per_batch": ms_predict, "atoms_per_s": (atoms / K) / (ms_predict * 1e-3),
+                                    "what": "nep_forward alone (E, F, virial of the batch; rank-local), back to back"},
                    "step_call": ("nep_train_step: one CUDA graph launch per step" if not use_dist else "nep_forward + nep_loss_grad + all-reduce + nep_adam_step"),
                    "kernel_events": f"{n_prof} extra steps after the timed region, through the three calls with CUDA events around every kernel", "setup_s": setup,
                    "device_bytes": nep.bytes_allocated, "parallelism": (f"dp{world}: {w.structures.n_struct} structures sharded by structure over the ranks (dataparallel.DataParallelNep: "
