@@ -220,3 +220,26 @@ def test_scaler_of_descriptors_is_inverse_range(small):
     assert s.shape == (model.D,)
     assert np.allclose(s, 1.0 / np.ptp(q, axis=0), rtol=1e-13)
     assert np.allclose((q * s).max(0) - (q * s).min(0), 1.0, rtol=1e-12)            # q~ spans exactly one unit (Eq. 2)
+
+
+@pytest.mark.parametrize("l3,l4,l5", [(1, 0, 1), (2, 2, 0), (3, 2, 1), (2, 0, 0)])
+def test_other_three_body_orders_are_row_subsets(small, l3, l4, l5):
+    """l_max = (l3, l4, l5) with l3 < 4 (Table I): the descriptor coefficients do not depend on l_max, so with the
+    same cR, cA every component the smaller model keeps must equal the same component of the (4, 2, 1) model, which the tests above pin
+    (addition theorem, scipy harmonics, Wigner-3j, cosine sums), in the row order of DESIGN C0:
+    radial n | 3-body (l, n), l = 1..l3 | 4-body n | 5-body n."""
+    model, st, th, q = small
+    sub = wl.ModelSpec(model.n_species, model.rc_R, model.rc_A, model.n_max_R, model.n_max_A, model.basis_R, model.basis_A, l3, l4, l5, model.neurons)
+    ths = np.zeros(sub.n_par)
+    a, b = model.block_slices(), sub.block_slices()
+    ths[b["cR"]] = th[a["cR"]]; ths[b["cA"]] = th[a["cA"]]
+    qs = O.descriptors(O.OracleData(sub, st), ths)
+    nR, nA = model.n_R, model.n_A
+    assert sub.D == nR + nA * (l3 + (l4 > 0) + (l5 > 0)) and qs.shape[1] == sub.D
+    rows = list(range(nR + l3 * nA))                                  # radial and l = 1..l3 sit at the same indices
+    if l4:
+        rows += list(range(nR + 4 * nA, nR + 5 * nA))                 # 4-body block of the (4, 2, 1) model
+    if l5:
+        rows += list(range(nR + 5 * nA, nR + 6 * nA))                 # 5-body block
+    assert np.allclose(qs, q[:, rows], rtol=0, atol=1e-13)
+    assert np.abs(qs).max() > 1e-3
