@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
     constexpr int NK = NCH * K, NKP = (NK + 3) & ~3;
     const int nwarp = blockDim.x >> 5;
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;
-    float* tab_all = smem + PAIR_TB * 16;                                           // [nwarp][NK]
+    float* tab_all = smem + PAIR_TB * 16;                                           // [NK] sums of the block, then the ticket of its warps
     const int n0 = blockIdx.y * NCH;
     const int wib = threadIdx.x >> 5;
     float* area = tab_all + (size_t)nwarp * NKP + (size_t)wib * staged_warp_floats(m, NCH);
@@ -29,6 +29,8 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
     if (STAGED && wg < (size_t)a.b.nbs)   // pass 0: tangent moments of the chunk and the angular rows of Qb
         rows_request(mbar, area, a.b.Sd + (wg * m.nA + n0) * NL * WARP, chunk_rows(m, n0, NCH),
                      area + NCH * NL * WARP, a.b.Qb + (wg * m.D + m.nR) * WARP, m.D - m.nR);
+    for (int i = threadIdx.x; i <= NKP; i += blockDim.x) tab_all[i] = 0.0f;           // (the ticket at [NKP] is an unsigned zero)
+    __syncthreads();
     Lane L;
     const bool inb = lane_init(a, L);
     constexpr int KH = (K + 1) / 2;
@@ -151,21 +153,28 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                 contract(B);
             });
         }
-        // every lane targets the same block of coefficients -> shuffle-reduce, lane 0 stores, block adds
+        // every lane targets the same block of coefficients: reduce-scatter over the lanes, then shared-memory adds into the block's table
+        constexpr int P = NK <= 32 ? 32 : (NK <= 64 ? 64 : 128), PL = P / 32;
+        float v[P];
 #pragma unroll
-        for (int n = 0; n < NCH; ++n)
+        for (int e = 0; e < P; ++e) v[e] = e < NK ? accv(e / K, e % K) : 0.0f;
+        warp_reduce_scatter<P>(v);
+        const int lane = threadIdx.x & 31;
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
-                const float v = warp_sum(accv(n, k));
-                if ((threadIdx.x & 31) == 0) tab_all[wib * NKP + n * K + k] = v;
-            }
-    } else {
-        for (int i = threadIdx.x & 31; i < NK; i += WARP) tab_all[wib * NKP + i] = 0.0f;
+        for (int j = 0; j < PL; ++j)
+            if (PL * lane + j < NK) atomicAdd(tab_all + PL * lane + j, v[j]);
     }
-    __syncthreads();
-    for (int i = threadIdx.x; i < NK; i += blockDim.x) {
-        float v = 0.0f;
-        for (int w = 0; w < nwarp; ++w) v += tab_all[w * NKP + i];
+    // no block barrier: a warp leaves when it is done; the last one of the block (ticket) adds the table to g
+    __syncwarp();
+    bool last = false;
+    if ((threadIdx.x & 31) == 0) {
+        __threadfence_block();
+        last = atomicAdd(reinterpret_cast<unsigned*>(tab_all + NKP), 1u) == (unsigned)nwarp - 1u;
+    }
+    if (!__shfl_sync(0xffffffffu, (int)last, 0)) return;
+    __threadfence_block();
+    for (int i = threadIdx.x & 31; i < NK; i += WARP) {
+        const float v = *reinterpret_cast<volatile float*>(tab_all + i);
         const int n = i / K, k = i - n * K;
         if (v != 0.0f && k < m.KA && n0 + n < m.nA) atomicAdd(a.g + m.o_cA + (size_t)(n0 + n) * m.KA + k, v);
     }

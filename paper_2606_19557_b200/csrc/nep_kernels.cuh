@@ -109,6 +109,25 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// Sum over the 32 lanes of P values per lane (P a power of two >= 32) in P - P/32 shuffles instead of 5 P: in each of the five steps a
+// lane keeps one half of its values and sends the other half to its partner.  Afterwards lane l holds, in v[0 .. P/32 - 1], the totals
+// of the elements (P/32) l .. (P/32) l + P/32 - 1.
+template <int P>
+__device__ __forceinline__ void warp_reduce_scatter(float* v)
+{
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int step = 0; step < 5; ++step) {
+        const int mask = 16 >> step, cnt = P >> (step + 1);
+        const bool up = lane & mask;
+#pragma unroll
+        for (int i = 0; i < cnt; ++i) {
+            const float keep = up ? v[i + cnt] : v[i], send = up ? v[i] : v[i + cnt];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
+        }
+    }
+}
+
 struct PairGeo {
     float dx, dy, dz, r, rinv, x, y, z;
     int jl, tj;
