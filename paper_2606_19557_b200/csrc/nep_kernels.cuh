@@ -456,8 +456,7 @@ __device__ __forceinline__ void load_Sbar(const StepArgs& a, const Lane& L, int 
             const bool on = ok && (s < 4 ? s < m.l3 : (s == 4 ? m.has4 : m.has5));
             cq[s] = on ? cq[s] : 0.0f; cf[s] = on ? cf[s] : 0.0f;
         }
-        inv_adjoint(S, cq, X[n]);
-        inv_hessian_action(S, Sd, cf, X[n]);
+        inv_adjoint_hessian(S, Sd, cq, cf, X[n]);
         if (!ok)
 #pragma unroll
             for (int l = 0; l < NL; ++l) X[n][l] = 0.0f;
@@ -501,8 +500,7 @@ __device__ __forceinline__ void load_Sbar_staged(const StepArgs& a, const Lane& 
             cq[s] = on ? Qs[(row * m.nA + nn) * WARP] : 0.0f;
             cf[n][s] = on ? cf[n][s] : 0.0f;
         }
-        inv_adjoint(S, cq, out);
-        inv_hessian_action(S, Sd, cf[n], out);
+        inv_adjoint_hessian(S, Sd, cq, cf[n], out);
 #pragma unroll
         for (int l = 0; l < NL; ++l) X[n][l] = ok ? out[l] : 0.0f;
     }

@@ -284,24 +284,29 @@ __device__ __forceinline__ void inv_tangent(const float* S, const float* V, floa
     qd[4] = 1.5f * KAPPA4 * sym_dot(T2, Td);
     qd[5] = 2.0f * C5 * lsum(S, 1) * qd[0];
 }
-// out[L] += sum_a c[a] sum_L' (d2 q_a / dS_L dS_L') V_L'
-__device__ __forceinline__ void inv_hessian_action(const float* S, const float* V, const float* c, float* out)
+// inv_adjoint(S, cq) plus the second-derivative action along V: out[L] = sum_a cq[a] dq_a/dS_L + sum_a cf[a] sum_L' (d2 q_a / dS_L dS_L') V_L'.
+// The two 4-body terms are 3 k4 cq4 T^2 and 3 k4 cf4 (T Td + Td T): both are anticommutators with T, so one anticommutator of T with
+// (cq4 / 2) T + cf4 Td (scaled by 3 k4) serves both.
+__device__ __forceinline__ void inv_adjoint_hessian(const float* S, const float* V, const float* cq, const float* cf, float* out)
 {
-    // d/dS_L [(28/15) q1 S_L] along V: (28/15) (q1d S_L + q1 V_L), q1d = 2 S.V
     const float q1 = lsum(S, 1), q1d = 2.0f * ldot(S, V, 1);
-    const float c1 = fmaf(4.0f * C5 * c[5], q1, 2.0f * c[0]);
-    const float c1s = 4.0f * C5 * c[5] * q1d;
+    const float a1 = fmaf(4.0f * C5 * cq[5], q1, 2.0f * cq[0]);          // coefficient of S_L, l = 1, from the first term
+    const float b1 = fmaf(4.0f * C5 * cf[5], q1, 2.0f * cf[0]);          // coefficient of V_L
+    const float a1s = fmaf(4.0f * C5 * cf[5], q1d, a1);                  // ... and of S_L from the second term
 #pragma unroll
-    for (int L = 0; L < 3; ++L) out[L] += fmaf(c1, V[L], c1s * S[L]);
+    for (int L = 0; L < 3; ++L) out[L] = fmaf(b1, V[L], a1s * S[L]);
 #pragma unroll
-    for (int L = 3; L < 8; ++L) out[L] = fmaf(2.0f * c[1], V[L], out[L]);
+    for (int L = 3; L < 8; ++L) out[L] = fmaf(2.0f * cf[1], V[L], 2.0f * cq[1] * S[L]);
 #pragma unroll
-    for (int L = 8; L < 15; ++L) out[L] = fmaf(2.0f * c[2], V[L], out[L]);
+    for (int L = 8; L < 15; ++L) out[L] = fmaf(2.0f * cf[2], V[L], 2.0f * cq[2] * S[L]);
 #pragma unroll
-    for (int L = 15; L < 24; ++L) out[L] = fmaf(2.0f * c[3], V[L], out[L]);
+    for (int L = 15; L < 24; ++L) out[L] = fmaf(2.0f * cf[3], V[L], 2.0f * cq[3] * S[L]);
     const Sym6 T = tensor_from_l2(S), Td = tensor_from_l2(V);
-    const Sym6 Pd = anticomm(T, Td);   // T Td + Td T ; d(3 k4 T^2) = 3 k4 (T Td + Td T)
-    l2_from_tensor_adjoint(Pd, 3.0f * KAPPA4 * c[4], out);
+    const float wq = 0.5f * cq[4], wf = cf[4];
+    Sym6 M;
+    M.xx = fmaf(wq, T.xx, wf * Td.xx); M.yy = fmaf(wq, T.yy, wf * Td.yy); M.zz = fmaf(wq, T.zz, wf * Td.zz);
+    M.xy = fmaf(wq, T.xy, wf * Td.xy); M.xz = fmaf(wq, T.xz, wf * Td.xz); M.yz = fmaf(wq, T.yz, wf * Td.yz);
+    l2_from_tensor_adjoint(anticomm(T, M), 3.0f * KAPPA4, out);
 }
 
 }  // namespace nep
