@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                 Prep P;
                 P.p = pair_geo(rc4);
                 P.fv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, false>(P.p.r, rcinv, [&](int k, float fk, float) { P.fv[k] = fk * on; });
+                cheb_basis<K, false>(P.p.r, rcinv, [&](int k, float fk, float) { P.fv[k] = fk; }, on);
                 return P;
             };
             auto contract = [&](const Prep& P) {
@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                 P.p = pair_geo(rc4);
                 P.T = pair_tangent(ub, bbase, P.p, uix, uiy, uiz, G);
                 P.fv[2 * KH - 1] = 0.0f; P.dfv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, true>(P.p.r, rcinv, [&](int k, float fk, float dfk) { P.fv[k] = fk * on; P.dfv[k] = dfk * on; });
+                cheb_basis<K, true>(P.p.r, rcinv, [&](int k, float fk, float dfk) { P.fv[k] = fk; P.dfv[k] = dfk; }, on);
                 return P;
             };
             auto contract = [&](const Prep& P) {

@@ -60,9 +60,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
     auto prep = [&](const float4& rc4, float on) {
         Prep P;
         P.p = pair_geo(rc4);
-        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, P.dg);
-#pragma unroll
-        for (int n = 0; n < NCH; ++n) { P.g[n] *= on; P.dg[n] *= on; }
+        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, P.dg, on);
         return P;
     };
     auto contract = [&](const Prep& P) {

@@ -93,9 +93,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
     auto prep = [&](const float4& rc4, float on) {
         Prep P;
         P.p = pair_geo(rc4);
-        radial_gn<NCH, K, false>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, nullptr);
-#pragma unroll
-        for (int n = 0; n < NCH; ++n) P.g[n] *= on;
+        radial_gn<NCH, K, false>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, nullptr, on);
         return P;
     };
     auto accumulate = [&](const Prep& P) {

@@ -54,9 +54,9 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
         P.p = pair_geo(rc4);
         P.T = pair_tangent(ub, bbase, P.p, uix, uiy, uiz, G);
         float dg[NCH];
-        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, dg);
+        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, dg, on);
 #pragma unroll
-        for (int n = 0; n < NCH; ++n) { P.g[n] *= on; P.c[n] = dg[n] * P.T.t * on; }
+        for (int n = 0; n < NCH; ++n) P.c[n] = dg[n] * P.T.t;
         return P;
     };
     // ... and the rank-1 update of the 5 x 24 tangent moments

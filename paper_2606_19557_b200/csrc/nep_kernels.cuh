@@ -343,7 +343,7 @@ __device__ __forceinline__ void coef_k(const float* __restrict__ cp, int k, floa
 
 // g_n(r) = sum_k c_nk f_k(r) (and g_n') for the chunk's channels  (Eq. 16)
 template <int NCH, int K, bool DERIV>
-__device__ __forceinline__ void radial_gn(float r, float rcinv, const float* __restrict__ cp, float* g, float* dg)
+__device__ __forceinline__ void radial_gn(float r, float rcinv, const float* __restrict__ cp, float* g, float* dg, float scale = 1.0f)
 {
 #pragma unroll
     for (int n = 0; n < NCH; ++n) { g[n] = 0.0f; if (DERIV) dg[n] = 0.0f; }
@@ -355,7 +355,7 @@ __device__ __forceinline__ void radial_gn(float r, float rcinv, const float* __r
             g[n] = fmaf(c[n], fk, g[n]);
             if (DERIV) dg[n] = fmaf(c[n], dfk, dg[n]);
         }
-    });
+    }, scale);
 }
 
 // descriptor rows of the angular invariants of channel n: slots 0..3 -> l = 1..4, slot 4 -> 4-body, slot 5 -> 5-body

@@ -56,19 +56,20 @@ __device__ __forceinline__ void sincospi_unit(float u, float& sn, float& cs)
 // constant (models with fewer functions run the next larger instantiation with zero-padded coefficients).
 // Without DERIV the derivative argument is 0 and its arithmetic is not generated.
 // ------------------------------------------------------------------------------------------------
+// scale multiplies every f_k and f_k' (they are linear in the three cutoff factors): a sweep masks a padded pair slot with scale = 0.
 template <int K, bool DERIV, class Body>
-__device__ __forceinline__ void cheb_basis(float r, float rcinv, Body&& body)
+__device__ __forceinline__ void cheb_basis(float r, float rcinv, Body&& body, float scale = 1.0f)
 {
     const float u = r * rcinv;
     float sn, cs;
     sincospi_unit(u, sn, cs);
-    const float hfc = fmaf(0.25f, cs, 0.25f);              // 1/2 f_c
+    const float hfc = fmaf(0.25f, cs, 0.25f) * scale;      // 1/2 f_c
     const float um1 = u - 1.0f;
     const float x = fmaf(2.0f * um1, um1, -1.0f);
     const float x2 = 2.0f * x;
     float hdfc = 0.0f, hdxfc = 0.0f;
     if (DERIV) {
-        hdfc = (-0.25f * PI_F) * rcinv * sn;               // 1/2 f_c'
+        hdfc = (-0.25f * PI_F) * rcinv * sn * scale;       // 1/2 f_c'
         hdxfc = 4.0f * um1 * rcinv * hfc;                  // 1/2 x' f_c
     }
     float T2 = 1.0f, T1 = x, dT2 = 0.0f, dT1 = 1.0f;
