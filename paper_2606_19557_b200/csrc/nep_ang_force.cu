@@ -1,6 +1,6 @@
 // nep_ang_force.cu -- S5 (angular part): the closed-form pair force of P:145 (DESIGN C8)
 //   p_ij = dE_i/dd_ij = sum_n sum_L EdS_nL [g_n'(r) b_L(r^) r^ + g_n(r) grad_d b_L(r^)],   EdS = dE_i/dS held in registers,
-// F_i += p_ij, F_j -= p_ij (one RED per component), W_s -= d_ij (x) p_ij.
+// F_i += p_ij, F_j -= p_ij (one vector RED per pair), W_s -= d_ij (x) p_ij.
 #include "nep_kernels.cuh"
 
 namespace nep {
@@ -93,9 +93,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
         const float py = fmaf(radial, p.y, (vy - vr * p.y) * p.rinv);
         const float pz = fmaf(radial, p.z, (vz - vr * p.z) * p.rinv);
         fx += px; fy += py; fz += pz;
-        const unsigned jb = (unsigned)(bbase + p.jl);
-        float* Fj = Fb + (size_t)(jb >> 5) * (3 * WARP) + (jb & 31);
-        atomicAdd(Fj, -px); atomicAdd(Fj + WARP, -py); atomicAdd(Fj + 2 * WARP, -pz);
+        force_add(Fb, (unsigned)(bbase + p.jl), -px, -py, -pz);
         w[0] = fmaf(-p.dx, px, w[0]); w[1] = fmaf(-p.dx, py, w[1]); w[2] = fmaf(-p.dx, pz, w[2]);
         w[3] = fmaf(-p.dy, px, w[3]); w[4] = fmaf(-p.dy, py, w[4]); w[5] = fmaf(-p.dy, pz, w[5]);
         w[6] = fmaf(-p.dz, px, w[6]); w[7] = fmaf(-p.dz, py, w[7]); w[8] = fmaf(-p.dz, pz, w[8]);
@@ -105,10 +103,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_force(StepArgs a)
         contract(A);
         if (has2) contract(B);
     });
-    if (L.ti >= 0) {
-        float* Fi = sb_ptr(Fb, L.w, 3, L.lane);
-        atomicAdd(Fi, fx); atomicAdd(Fi + WARP, fy); atomicAdd(Fi + 2 * WARP, fz);
-    }
+    if (L.ti >= 0) force_add(Fb, L.ib, fx, fy, fz);
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
         const float v = warp_sum(w[k]);

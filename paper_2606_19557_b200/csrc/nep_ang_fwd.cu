@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
         // the structure accumulators that the force sweeps add into start from zero (benign duplicate stores)
         if (L.lane < 9) a.b.Ws[9 * L.sb + L.lane] = 0.0f;
         else if (L.lane == 9) a.b.Es[L.sb] = 0.0;
+        reinterpret_cast<float4*>(a.b.F)[L.ib] = make_float4(0.f, 0.f, 0.f, 0.f);   // both force sweeps add into F
         if (!STAGED) radial_descriptors(sb_ptr(a.d.B, L.ds, TK, L.lane));
     }
 

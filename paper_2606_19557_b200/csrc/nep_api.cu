@@ -570,7 +570,7 @@ static int ensure_batch_capacity(nep_ctx* c, int64_t NBP, int Sb, int nbs, int64
         ALLOC(c, b.S, float, n * m.nA * 24); ALLOC(c, b.Sd, float, n * m.nA * 24);
         ALLOC(c, b.qd, float, n * m.D);  ALLOC(c, b.Qb, float, n * m.D);
         ALLOC(c, b.arow, float, n * m.T * m.KRP); ALLOC(c, b.Bd, float, n * m.T * m.KR);
-        ALLOC(c, b.F, float, n * 3);     ALLOC(c, b.u, float, n * 3);     ALLOC(c, b.Ei, float, n);
+        ALLOC(c, b.F, float, n * 4);     ALLOC(c, b.u, float, n * 3);     ALLOC(c, b.Ei, float, n);
         c->cap_NBP = NBP;
     }
     if (tiles_m > c->cap_tiles_m) {

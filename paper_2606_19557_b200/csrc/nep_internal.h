@@ -57,6 +57,7 @@ struct DataDev {
     // sliced pair cache: record (slice, slot s, lane) at rec[recoff[slice] + s*32 + lane]
     const int* cntR; const int64_t* recoffR; const float4* recR;
     const int* cntA; const int64_t* recoffA; const float4* recA;
+    const int* cntH; const int64_t* recoffH; const float4* recH;   // half list of the radial pairs (one record per undirected pair; nep_neighbor.cu)
     const float* B;        // [nslices][T*KR][32] radial aggregate  B_k[T'] = sum_{j in N_R(i), t_j = T'} f_k(r_ij)
 };
 
@@ -88,7 +89,7 @@ struct BatchDev {
     float* hbuf;   // [ntiles][HP][tile_m] tanh outputs, tile order
     float* arow;   // [NBP][T*KRP]   a_k[T'] = sum_n Fp_n cR[t_i][T'][n][k]
     float* Bd;     // [nbs][T*KR][32] tangent of B
-    float* F;      // [nbs][3][32]
+    float* F;      // [NBP][4]  (F_x, F_y, F_z, unused) per batch-padded atom: one 16-byte cell, scattered to with vector REDs
     float* u;      // [nbs][3][32]   dL/dF
     float* Ei;     // [nbs][32]
     // per structure

@@ -128,6 +128,14 @@ __device__ __forceinline__ void warp_reduce_scatter(float* v)
     }
 }
 
+// Forces of the batch: F[batch-padded atom][4] = (F_x, F_y, F_z, unused), one 16-byte cell per atom, so that a scattered pair
+// reaction is ONE vector reduction (red.global.add.v4.f32) instead of three scalar ones: a warp-wide scatter costs the SM's
+// load/store path ~41 cycles per instruction whatever its width.
+__device__ __forceinline__ void force_add(float* F, unsigned ib, float x, float y, float z)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(F + 4 * (size_t)ib), "f"(x), "f"(y), "f"(z), "f"(0.0f) : "memory");
+}
+
 struct PairGeo {
     float dx, dy, dz, r, rinv, x, y, z;
     int jl, tj;

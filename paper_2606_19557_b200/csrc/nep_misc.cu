@@ -23,13 +23,14 @@ __global__ void __launch_bounds__(256) k_loss(StepArgs a, float lamE, float lamF
         const int w = (int)(ia >> 5), lane = (int)(ia & 31);
         const int4 bi = __ldg(a.b.binfo + w);
         const float c = (float)(2.0 * dlamF / (3.0 * a.b.nrmN));
-        const float* Fp = sb_ptr(a.b.F, w, 3, lane);
+        const float4 F4 = reinterpret_cast<const float4*>(a.b.F)[ia];
+        const float Fp[3] = { F4.x, F4.y, F4.z };
         const float* Fl = sb_ptr(a.d.Flab, bi.x, 3, lane);
         float* up = sb_ptr(a.b.u, w, 3, lane);
         float s2 = 0.0f;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const float dF = Fp[k * WARP] - __ldg(Fl + k * WARP);   // padding slots hold 0 in both (no type lookup on this path)
+            const float dF = Fp[k] - __ldg(Fl + k * WARP);   // padding slots hold 0 in both (no type lookup on this path)
             s2 = fmaf(dF, dF, s2);
             up[k * WARP] = c * dF;
         }
@@ -156,8 +157,8 @@ __global__ void k_gather_outputs(StepArgs a, float* E, float* F, float* W)
         const int il = a.d.orig_p[(size_t)bi.x * WARP + lane];
         if (il >= 0) {
             const int64_t o = a.b.bfoff[bi.y] + il;
-            const float* Fp = sb_ptr(a.b.F, w, 3, lane);
-            F[3 * o] = Fp[0]; F[3 * o + 1] = Fp[WARP]; F[3 * o + 2] = Fp[2 * WARP];
+            const float4 F4 = reinterpret_cast<const float4*>(a.b.F)[i];
+            F[3 * o] = F4.x; F[3 * o + 1] = F4.y; F[3 * o + 2] = F4.z;
         }
     }
 }

@@ -263,6 +263,48 @@ __global__ void k_cache_fill(int nslices, ModelDev m, const double* __restrict__
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Half list of the radial pairs (one record per UNDIRECTED pair) for the radial force sweep: the pair (i, j, n) and its mirror
+// (j, i, -n) share f_k'(r), so one thread evaluates the basis once, forms s_ij + s_ji and scatters the reaction to j.
+// Owner of a pair: for i != j the atom with the smaller slot if i + j is odd, the larger one if it is even (every atom keeps about
+// half of its pairs); a self-image pair (i, i, n) is kept for the image whose bond vector is lexicographically positive (its mirror
+// has exactly the negated vector).  Records keep their order (sorted by neighbour type).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool owns_pair(int i, const float4& rec)
+{
+    const int j = __float_as_int(rec.w) & 0xffffff;
+    if (j != i) return ((i + j) & 1) ? (i < j) : (i > j);
+    return rec.x > 0.0f || (rec.x == 0.0f && (rec.y > 0.0f || (rec.y == 0.0f && rec.z > 0.0f)));
+}
+template <bool FILL>
+__global__ void k_half_list(int nslices, const int64_t* __restrict__ pbase, const int* __restrict__ slice_struct, const int* __restrict__ cnt,
+                            const int64_t* __restrict__ recoff, const float4* __restrict__ rec, int* __restrict__ cntH, int* __restrict__ widthH,
+                            const int64_t* __restrict__ recoffH, float4* __restrict__ recH)
+{
+    const int sl = (int)((blockIdx.x * blockDim.x + threadIdx.x) / WARP), lane = threadIdx.x & 31;
+    if (sl >= nslices) return;
+    const int64_t ip = (int64_t)sl * WARP + lane;
+    const int i = (int)(ip - pbase[slice_struct[sl]]);
+    const int n = cnt[ip];
+    const float4* r4 = rec + recoff[sl] + lane;
+    float4* out = FILL ? recH + recoffH[sl] + lane : nullptr;
+    int c = 0;
+    for (int s = 0; s < n; ++s) {
+        const float4 r = r4[(int64_t)s * WARP];
+        if (owns_pair(i, r)) {
+            if (FILL) out[(int64_t)c * WARP] = r;
+            ++c;
+        }
+    }
+    if (!FILL) {
+        cntH[ip] = c;
+        int w = c;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) w = max(w, __shfl_xor_sync(0xffffffffu, w, o));
+        if (lane == 0) widthH[sl] = w;
+    }
+}
+
 static int scan_excl(nep_ctx* c, const int* in, int64_t* out, int64_t n, int mult)
 {
     prof_begin(c, "k_scan_excl");
@@ -284,10 +326,12 @@ int build_neighbors_dev(nep_ctx* c)
     const int64_t N = c->N;
     // release lists of a previous build
     {
-        const void* ptrs[] = { d.offR, d.jR, d.shR, d.offA, d.jA, d.shA, d.cntR, d.recoffR, d.recR, d.cntA, d.recoffA, d.recA, d.B };
+        const void* ptrs[] = { d.offR, d.jR, d.shR, d.offA, d.jA, d.shA, d.cntR, d.recoffR, d.recR, d.cntA, d.recoffA, d.recA, d.B,
+                               d.cntH, d.recoffH, d.recH };
         for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
         d.offR = d.offA = nullptr; d.jR = d.jA = nullptr; d.shR = d.shA = nullptr; d.cntR = d.cntA = nullptr;
         d.recoffR = d.recoffA = nullptr; d.recR = d.recA = nullptr; d.B = nullptr;
+        d.cntH = nullptr; d.recoffH = nullptr; d.recH = nullptr;
         c->have_nbrs = false;
     }
     // ---- host: cell geometry per structure ----
@@ -423,8 +467,25 @@ int build_neighbors_dev(nep_ctx* c)
                                                  offA, jA, shA, recoffA, recA, nullptr, c->NP);
     prof_end(c);
     NEP_CUDA(c, cudaGetLastError());
+    // half list of the radial pairs
+    DALLOC(cntHp, int, c->NP); DALLOC(wH, int, ns); DALLOC(recoffH, int64_t, ns + 1);
+    prof_begin(c, "k_half_list");
+    k_half_list<false><<<gS, TB, 0, c->stream>>>(ns, d.pbase, d.slice_struct, cntRp, recoffR, recR, cntHp, wH, nullptr, nullptr);
+    prof_end(c);
+    if ((rc = scan_excl(c, wH, recoffH, ns, WARP))) return rc;
+    int64_t totH = 0;
+    NEP_CUDA(c, cudaMemcpyAsync(&totH, recoffH + ns, 8, cudaMemcpyDeviceToHost, c->stream));
     NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    DALLOC(recH, float4, totH);
+    NEP_CUDA(c, cudaMemsetAsync(recH, 0, 16 * (size_t)std::max<int64_t>(totH, 1), c->stream));
+    prof_begin(c, "k_half_list");
+    k_half_list<true><<<gS, TB, 0, c->stream>>>(ns, d.pbase, d.slice_struct, cntRp, recoffR, recR, nullptr, nullptr, recoffH, recH);
+    prof_end(c);
+    NEP_CUDA(c, cudaGetLastError());
+    NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+    dev_free(c, wH);
     d.cntR = cntRp; d.cntA = cntAp; d.recoffR = recoffR; d.recoffA = recoffA; d.recR = recR; d.recA = recA; d.B = B;
+    d.cntH = cntHp; d.recoffH = recoffH; d.recH = recH;
     void* temps[] = { d_cg, d_as, d_cell_of, d_cell_cnt, d_cell_fill, d_cell_start, d_cell_atoms, d_cR, d_cA, keys, wR, wA };
     for (void* p : temps) dev_free(c, p);
     return NEP_OK;

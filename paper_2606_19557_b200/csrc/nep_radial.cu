@@ -1,7 +1,9 @@
 // nep_radial.cu -- the two sweeps over the radial pair list.
-// S5 (radial part): F_i = sum_j (s_ij + s_ji) r^_ij with s_ij = sum_k a^i_k[t_j] f_k'(r_ij), a^i_k[T'] = sum_n Fp_n cR[t_i][T'][n][k];
-//     the reverse pair's coefficient row a^j[t_i] is gathered (rows of one structure are cache resident): no atomics,
-//     deterministic.  W_s -= sum d (x) (s_ij r^).  Also folds the per-atom energies into E_s (Eq. 1).
+// S5 (radial part): F_i = sum_j (s_ij + s_ji) r^_ij with s_ij = sum_k a^i_k[t_j] f_k'(r_ij), a^i_k[T'] = sum_n Fp_n cR[t_i][T'][n][k].
+//     The sweep walks the HALF list (one record per undirected pair, nep_neighbor.cu): the pair and its mirror share f_k'(r), so the
+//     owner evaluates the basis once, gathers the other atom's coefficient row a^j[t_i] (rows of one structure are cache resident),
+//     adds (s_ij + s_ji) r^ to its own force and scatters the reaction to j (one vector RED, like the angular force sweep).
+//     W_s -= sum d (x) ((s_ij + s_ji) r^).  Also folds the per-atom energies into E_s (Eq. 1).
 // S7 (radial part): Bd_k[T'] = sum_{j, t_j = T'} f_k'(r_ij) (r^_ij . d~_ij), the tangent of the aggregate B (DESIGN C10).
 #include "nep_kernels.cuh"
 
@@ -37,7 +39,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
     Lane L;
     if (!lane_init(a, L)) return;
     const ModelDev& m = a.m;
-    const SweepA sw = sweep_init(a.d.recoffR, a.d.recR, a.d.cntR, L);
+    const SweepA sw = sweep_init(a.d.recoffH, a.d.recH, a.d.cntH, L);
     constexpr int KP = (K + 3) & ~3;
     const int KRP = m.KRP, TKRP = m.T * m.KRP;
     float ai[KP];
@@ -47,6 +49,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
     float fx = 0.f, fy = 0.f, fz = 0.f, wxx = 0.f, wyy = 0.f, wzz = 0.f, wxy = 0.f, wxz = 0.f, wyz = 0.f;
     const float* arow = a.b.arow;
     const float* arow_i = arow + (size_t)L.ib * TKRP;
+    float* Fb = a.b.F;
     const int ti = L.ti, bbase = L.bbase;
     const float rcinv = m.rcinvR;
     auto one = [&](const float4& rc4) {
@@ -72,8 +75,9 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
             sji = fmaf(aj[k], dfk, sji);
         });
         const float fs = sij + sji;
-        fx = fmaf(fs, p.x, fx); fy = fmaf(fs, p.y, fy); fz = fmaf(fs, p.z, fz);
-        const float px = sij * p.x, py = sij * p.y, pz = sij * p.z;
+        const float px = fs * p.x, py = fs * p.y, pz = fs * p.z;
+        fx += px; fy += py; fz += pz;
+        force_add(Fb, (unsigned)(bbase + p.jl), -px, -py, -pz);
         wxx = fmaf(-p.dx, px, wxx); wyy = fmaf(-p.dy, py, wyy); wzz = fmaf(-p.dz, pz, wzz);
         wxy = fmaf(-p.dx, py, wxy); wxz = fmaf(-p.dx, pz, wxz); wyz = fmaf(-p.dy, pz, wyz);
     };
@@ -81,8 +85,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
         one(ra);
         if (has2) one(rb);
     });
-    float* Fi = sb_ptr(a.b.F, L.w, 3, L.lane);
-    Fi[0] = fx; Fi[WARP] = fy; Fi[2 * WARP] = fz;
+    if (L.ti >= 0) force_add(Fb, L.ib, fx, fy, fz);   // F was cleared by k_ang_fwd
     wxx = warp_sum(wxx); wyy = warp_sum(wyy); wzz = warp_sum(wzz); wxy = warp_sum(wxy); wxz = warp_sum(wxz); wyz = warp_sum(wyz);
     const double Es = warp_sum(L.ti >= 0 ? (double)a.b.Ei[L.ib] : 0.0);
     if (L.lane == 0) {

@@ -39,8 +39,9 @@ def kernel_models(model, sizes: dict) -> dict:
                           bytes=16 * PA + N * f4 * (NL * nA + nA * nang) + N * f4 * (T * KR + nR))
     m["k_ann_fwd"] = dict(flops=N * (4 * H * D + 6 * H + 2 * D + 2 * T * nR * KR),
                           bytes=N * f4 * (2 * D + H + T * KRP + 1))
-    m["k_rad_force"] = dict(flops=PR * (GEO + basisd(KR) + 4 * KR + 22),
-                            bytes=16 * PR + N * f4 * (T * KRP + 3))
+    # half list: one record per undirected pair; both directions' sums s_ij, s_ji from one evaluation of the basis
+    m["k_rad_force"] = dict(flops=(PR // 2) * (GEO + basisd(KR) + 4 * KR + 30),
+                            bytes=16 * (PR // 2) + N * f4 * (T * KRP + 3))
     m["k_ang_force"] = dict(flops=PA * (GEO + basisd(KA) + 4 * nA * KA + Y + nA * (4 * NL + 2) + GRADC + 14 + 24),
                             bytes=16 * PA + N * f4 * (NL * nA + nA * nang + 3))
     m["k_rad_tangent"] = dict(flops=PR * (GEO + PTAN + basisd(KR) + 2 * KR),
