@@ -145,7 +145,8 @@ int nep_compute_descriptor_range(nep_ctx* ctx, double* qmin, double* qmax);
 int nep_set_scaler_from_range(nep_ctx* ctx, const double* qmin, const double* qmax);
 
 /* Mini-batch = a list of structure ids ("batch" of Table I).  ids == NULL: the whole set.
- * ids are copied to the device; the same id must not appear twice. */
+ * ids are copied to the device; the same id must not appear twice.  Selecting the batch that is already current (full-batch
+ * training does so every step) uploads its tables again but keeps the tables derived from them on the device. */
 int nep_set_batch(nep_ctx* ctx, int n, const int* struct_ids);
 
 /* S1-S5: descriptors, network, energies (Eq. 1), forces and virials (P:145 closed forms) of the batch.

@@ -78,6 +78,7 @@ namespace nep {
 // every slot and the slot of every atom; the force labels follow if they are loaded.
 int upload_slot_tables(nep_ctx* c)
 {
+    c->batch_tables_valid = false;     // the type-sorted atom list of a batch depends on the slot order
     DataDev& d = c->d;
     const int T = c->m.T;
     std::vector<int> type_p((size_t)c->NP, -1), rank_p((size_t)c->NP, 0), orig_p((size_t)c->NP, -1);
@@ -202,6 +203,7 @@ static void free_dataset(nep_ctx* c)
     for (const void* p : ptrs) dev_free(c, const_cast<void*>(p));
     memset(&d, 0, sizeof d);
     c->have_data = c->have_labels = c->have_nbrs = c->forward_valid = c->grad_valid = c->loss_valid = false;
+    c->batch_tables_valid = false;
     ++c->graph_gen;
 }
 
@@ -329,6 +331,7 @@ int nep_build_neighbors(nep_ctx* c)
 {
     CHECK_CTX(c);
     if (!c->have_data) return fail(c, NEP_ESTATE, "nep_build_neighbors before nep_load_structures");
+    c->batch_tables_valid = false;
     int rc = build_neighbors_dev(c);
     if (rc) return rc;
     c->have_nbrs = true;
@@ -615,6 +618,22 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
     if (ids && n < 0) return fail(c, NEP_EINVAL, "negative batch size");
     const int Sb = ids ? n : c->S;
     const int T = c->m.T;
+    // The same batch as the current one (full-batch training re-selects it every step): the tables in the pinned block and the
+    // type-sorted atom list on the device are still those of this batch; only the upload is repeated.
+    if (c->batch_tables_valid && Sb == c->b.Sb && Sb > 0 && (int)c->h_bsid.size() == Sb) {
+        bool same = true;
+        for (int k = 0; k < Sb && same; ++k) same = c->h_bsid[k] == (ids ? ids[k] : k);
+        if (same) {
+            const size_t bytes = 16 * (size_t)c->b.nbs + 8 * (size_t)Sb + 4 * (size_t)Sb * (2 + T);
+            NEP_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, bytes, cudaMemcpyHostToDevice, c->stream));
+            c->forward_valid = c->grad_valid = false;
+            const double nS = (double)c->b.Sb, nN = (double)c->b.Nb, nV = (double)c->b.Sv;              // as after any nep_set_batch
+            if (c->b.nrmS != nS || c->b.nrmN != nN || c->b.nrmV != nV) ++c->graph_gen;
+            c->b.nrmS = nS; c->b.nrmN = nN; c->b.nrmV = nV;
+            return NEP_OK;
+        }
+    }
+    c->batch_tables_valid = false;
     std::vector<unsigned char> seen(ids ? c->S : 0, 0);
     int64_t nbs64 = 0;
     for (int k = 0; k < Sb; ++k) {
@@ -680,7 +699,9 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
     c->h_bsid.assign(bsid, bsid + Sb); c->h_bfoff.assign(bfoff, bfoff + Sb); c->PRb = PRb; c->PAb = PAb;
     c->forward_valid = c->grad_valid = false;
     if (memcmp(&b_before, &c->b, sizeof(BatchDev)) != 0) ++c->graph_gen;
-    return launch_build_alist(c);
+    rc = launch_build_alist(c);
+    c->batch_tables_valid = rc == NEP_OK;
+    return rc;
 }
 
 static int copy_out(nep_ctx* c, void* dst, const float* src, size_t count, int on_host)

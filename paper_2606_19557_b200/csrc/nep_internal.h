@@ -140,6 +140,7 @@ struct nep_ctx {
     nep::BatchDev b{};
     int64_t cap_NBP = 0; int cap_Sb = 0; int cap_nbs = 0; int64_t cap_tiles_m = 0;
     std::vector<int> h_bsid; std::vector<int64_t> h_bfoff;
+    bool batch_tables_valid = false;   // the pinned block and the device tables hold the tables of batch h_bsid (nep_set_batch fast path)
     int64_t PRb = 0, PAb = 0;
     std::vector<int64_t> h_pairsR_struct, h_pairsA_struct;   // pairs per structure (for sizes / flop models)
     // pinned staging for the per-batch tables (one async copy per nep_set_batch)

@@ -112,6 +112,42 @@ def test_mini_batches(name):
         H.check_forward(nep, prob)
 
 
+def test_same_batch_selected_again():
+    """nep_set_batch with the ids of the current batch re-uploads the tables but keeps the derived device tables: results, the reset of
+    the whole-batch normalisers and the step graph behave as after any nep_set_batch."""
+    prob = _prob("cfg3")
+    S = prob.workload.structures.n_struct
+    ids = np.random.default_rng(3).permutation(S)[: S - 2]
+    lam = (1.0, 2.0, 3.0)
+    l4o, go = O.loss_grad(prob.data, prob.theta, prob.scaler, lam, batch=list(ids))
+    with H.make_gpu(prob) as nep:
+        nep.set_batch(ids)
+        nep.set_batch(ids)                                   # fast path
+        H.check_forward(nep, prob, batch=ids)
+        H.check_grad(nep, prob, lam, batch=ids)
+        nat = prob.workload.structures.n_atoms
+        nep.set_batch_normalisers(2 * len(ids), 2 * int(nat[ids].sum()), 2 * len(ids))
+        nep.forward(want=())
+        half = nep.loss_grad(*lam)
+        assert np.allclose(half, 0.5 * l4o, rtol=2e-4)       # counts of a batch twice as large: every mean halves
+        nep.set_batch(ids)                                   # the local counts again
+        nep.forward(want=())
+        assert np.allclose(nep.loss_grad(*lam), l4o, rtol=2e-4)
+        nep.set_batch(ids[::-1].copy())                      # another order is another batch
+        H.check_forward(nep, prob, batch=ids[::-1])
+        th0 = nep.get_params()
+        for _ in range(3):                                   # stepping through the graph with the batch re-selected every step
+            nep.set_batch(ids)
+            nep.train_step(*lam, 1e-3, use_graph=True)
+        th_a = nep.get_params()
+        nep.set_params(th0); nep.set_adam_state(np.zeros_like(th0), np.zeros_like(th0), np.zeros_like(th0), 0)
+        nep.set_batch(ids)
+        for _ in range(3):
+            nep.train_step(*lam, 1e-3, use_graph=False)
+        th_b = nep.get_params()
+        assert np.linalg.norm(th_a - th_b) <= 1e-3 * np.linalg.norm(th_a - th0)     # same trajectory up to the order of atomic sums
+
+
 def test_empty_batch_and_state_errors():
     from paper_2606_19557_b200.binding import NepError, NEP_ESTATE, NEP_EINVAL
     prob = _prob("tiny_T2")
