@@ -156,6 +156,7 @@ int nep_create(nep_ctx** out, int n_species, double rc_R, double rc_A, int n_max
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&c->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&c->max_smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    if (cudaMallocHost(&c->h_small, sizeof c->h_small_bytes) != cudaSuccess) { c->h_small = nullptr; cudaGetLastError(); }
     {   // network kernels: tensor-core tiles when they fit; NEP_ANN_FFMA=1 selects the FFMA tiles (measurement aid)
         const char* e = getenv("NEP_ANN_FFMA");
         c->ann_tc = !(e && e[0] == '1') && ann_tc_fits(c, false) && ann_tc_fits(c, true);
@@ -186,6 +187,7 @@ int nep_destroy(nep_ctx* c)
     std::vector<void*> a = c->allocs;
     for (void* p : a) dev_free(c, p);
     if (c->h_stage) cudaFreeHost(c->h_stage);
+    if (c->h_small) cudaFreeHost(c->h_small);
     for (auto& r : c->prof.pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto e : c->prof.pool) cudaEventDestroy(e);
     delete c;
@@ -361,6 +363,12 @@ static int h2d(nep_ctx* c, void* dst, const void* src, size_t bytes)
 }
 static int d2h(nep_ctx* c, void* dst, const void* src, size_t bytes)
 {
+    if (bytes <= sizeof c->h_small_bytes && c->h_small) {   // small results (the loss terms) through a pinned bounce buffer
+        NEP_CUDA(c, cudaMemcpyAsync(c->h_small, src, bytes, cudaMemcpyDeviceToHost, c->stream));
+        NEP_CUDA(c, cudaStreamSynchronize(c->stream));
+        memcpy(dst, c->h_small, bytes);
+        return NEP_OK;
+    }
     NEP_CUDA(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
     NEP_CUDA(c, cudaStreamSynchronize(c->stream));
     return NEP_OK;

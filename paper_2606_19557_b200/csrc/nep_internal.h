@@ -145,6 +145,7 @@ struct nep_ctx {
     std::vector<int64_t> h_pairsR_struct, h_pairsA_struct;   // pairs per structure (for sizes / flop models)
     // pinned staging for the per-batch tables (one async copy per nep_set_batch)
     void* h_stage = nullptr; size_t h_stage_bytes = 0; void* d_stage = nullptr; size_t d_stage_bytes = 0;
+    void* h_small = nullptr; char h_small_bytes[64];   // pinned bounce buffer (and its size) for small device -> host results
 
     float *theta = nullptr, *g = nullptr, *am = nullptr, *av = nullptr, *avmax = nullptr, *scaler = nullptr;
     float* qrange = nullptr;   // [2][DP] per-component minimum and maximum of the descriptors (S0c)
