@@ -185,6 +185,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
 // run of neighbour type t ends it stores a SNAPSHOT of them (12 x 128-bit stores into its own row of a lane-major table
 // snap[lane][t][n k], row stride an odd number of 16-byte units: conflict free); types the lane does not meet get the snapshot
 // of the type before them, so that the sum over the pairs with neighbour type t is snap[t] - snap[t - 1] for every lane.
+// The last type's snapshot is the final state of the accumulators and stays in registers.
 // After the sweep the lanes of one centre type are a contiguous range (slot order of a slice): thread r sums column
 // r = (t, n, k) over that range and issues one RED per (t_i, t_j, n, k).
 // ------------------------------------------------------------------------------------------------
@@ -195,7 +196,8 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
     const ModelDev& m = a.m;
     constexpr int NK = NCH * K, NKP = (NK + 3) & ~3, KH = (K + 1) / 2;
     const int T = m.T;
-    const int LS = (T * NKP) + (((T * NKP) >> 2) & 1 ? 0 : 4);          // lane stride (words): LS / 4 odd
+    const int TR = T - 1;                                               // table rows per lane: the last type is never stored (below)
+    const int LS = (TR * NKP) + (((TR * NKP) >> 2) & 1 ? 0 : 4);        // lane stride (words): LS / 4 odd
     float4* stage = reinterpret_cast<float4*>(smem) + threadIdx.x;      // SWEEP_STAGES cells per thread, WARP apart
     float* tab = smem + (WARP * 4 * SWEEP_STAGES);
     const int n0 = blockIdx.y * NCH;
@@ -218,8 +220,9 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
     auto accv = [&](int e) -> float { const int n = e / K, k = e - n * K; return e < NK ? ((k & 1) ? acc2[n][k >> 1].y : acc2[n][k >> 1].x) : 0.0f; };
     float* mine = tab + (size_t)lane * LS;
     int cur = 0;
-    auto snapshot_to = [&](int tj) {      // rows cur .. tj - 1 <- the accumulators as they are
-        while (cur < tj) {
+    auto snapshot_to = [&](int tj) {      // rows cur .. tj - 1 <- the accumulators as they are (row T - 1 would hold the final values: not stored)
+        const int end = tj < TR ? tj : TR;
+        while (cur < end) {
             float4* dst = reinterpret_cast<float4*>(mine + cur * NKP);
 #pragma unroll
             for (int i = 0; i < NKP / 4; ++i) dst[i] = make_float4(accv(4 * i), accv(4 * i + 1), accv(4 * i + 2), accv(4 * i + 3));
@@ -311,8 +314,12 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
     // Column sums per centre type: the lanes of one type are a contiguous range.  A thread owns QUADS of four consecutive
     // table columns (t_j, 4 e .. 4 e + 3) and walks the lanes of the range with one 128-bit load each; the sums of neighbour
     // type t_j are snapshot differences, taken through a small array of the column sums.
-    const int nquad = (T * NKP) >> 2;
+    // The snapshot of the LAST neighbour type is the final state of the accumulators, which every lane still holds in registers: its
+    // column sums come from a masked reduce-scatter over the lanes instead of a table row (one row per lane less: 25 instead of 31 KB of
+    // shared memory per warp at five species, 8 instead of 6 warps per SM).
+    const int nquad = (TR * NKP) >> 2;
     float* cs = tab + (size_t)WARP * LS;                 // [T * NKP] column sums of the current centre type
+    constexpr int P = NK <= 32 ? 32 : (NK <= 64 ? 64 : 128), PL = P / 32;
     const size_t tstep = (size_t)T * m.nA * m.KA;
     for (int ti = 0; ti < T; ++ti) {
         const unsigned bm = __ballot_sync(0xffffffffu, L.ti == ti);
@@ -326,6 +333,16 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
                 v.x += x.x; v.y += x.y; v.z += x.z; v.w += x.w;
             }
             *reinterpret_cast<float4*>(cs + 4 * qd) = v;
+        }
+        {
+            const bool in = lane >= c0 && lane < c1;
+            float v[P];
+#pragma unroll
+            for (int e = 0; e < P; ++e) v[e] = in ? accv(e) : 0.0f;
+            warp_reduce_scatter<P>(v);
+#pragma unroll
+            for (int j = 0; j < PL; ++j)
+                if (PL * lane + j < NKP) cs[TR * NKP + PL * lane + j] = v[j];
         }
         __syncwarp();
         for (int r = lane; r < T * NKP; r += WARP) {
@@ -362,7 +379,7 @@ int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
             }
         } else {
             constexpr int NKP = (NK + 3) & ~3;
-            const int LS = (m.T * NKP) + ((((m.T * NKP) >> 2) & 1) ? 0 : 4);
+            const int LS = ((m.T - 1) * NKP) + (((((m.T - 1) * NKP) >> 2) & 1) ? 0 : 4);
             const size_t smem = (size_t)WARP * 16 * SWEEP_STAGES + 4 * ((size_t)WARP * LS + (size_t)m.T * NKP);
             if (smem > (size_t)c->max_smem_optin) return fail(c, NEP_ECAPACITY, "angular coefficient tables do not fit in shared memory");
             auto kern = k_ang_adjoint_ms<NCH, K>;
