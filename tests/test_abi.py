@@ -54,7 +54,21 @@ def test_create_without_gpu_fails_loudly_or_validates(built):
         assert rc == binding.NEP_EINVAL and b"l_max" in L.nep_last_error(None)
     rc = L.nep_create_from_model_file(ctypes.byref(h), b"/nonexistent/model.txt", null_a, null_f, None, None)
     assert rc == binding.NEP_EINVAL and b"cannot open" in L.nep_last_error(None)
+    import os
+    import tempfile
     import torch
+    with tempfile.TemporaryDirectory() as td:               # the model-file reader runs on the host: header checks need no device
+        bad = os.path.join(td, "bad.txt")
+        open(bad, "w").write("nep_b200_model 2\nn_species 1\n")
+        rc = L.nep_create_from_model_file(ctypes.byref(h), bad.encode(), null_a, null_f, None, None)
+        assert rc == binding.NEP_EINVAL and b"not a nep_b200 model file" in L.nep_last_error(None)
+        good = os.path.join(td, "good.txt")
+        open(good, "w").write("nep_b200_model 1\nn_species 1\ncutoff 3 2\nn_max 0 0\nbasis_size 1 1\nl_max 4 0 0\nneuron 1\n"
+                              "scaler 5\n1\n1\n1\n1\n1\ntheta 12\n" + "0.5\n" * 12)
+        rc = L.nep_create_from_model_file(ctypes.byref(h), good.encode(), null_a, null_f, None, None)
+        # a well-formed header reaches nep_create: without a device that is NEP_ECUDA, with one the NULL allocator is refused
+        assert rc == (binding.NEP_EINVAL if torch.cuda.is_available() else binding.NEP_ECUDA)
+        assert b"not a nep_b200 model file" not in L.nep_last_error(None)
     if not torch.cuda.is_available():
         rc = L.nep_create(ctypes.byref(h), 1, 5.0, 4.0, 4, 4, 8, 8, 4, 2, 1, 30, null_a, null_f, None, None)
         assert rc == binding.NEP_ECUDA and b"no CPU fallback" in L.nep_last_error(None)
