@@ -26,6 +26,11 @@ def _cases():
         "tiny_l3_2_4body": lambda: wl.tiny_workload(9, model=wl.ModelSpec(2, 3.2, 2.8, 1, 3, 2, 4, 2, 2, 0, 6)),
         "tiny_l3_3_full": lambda: wl.tiny_workload(10, n_species=3, sizes=(33, 2, 40), box=(7.5, 3.1, 8.0),
                                                    model=wl.ModelSpec(3, 3.2, 2.6, 2, 5, 3, 4, 3, 2, 1, 7)),
+        # the largest basis (17 functions: the K = 17 instantiations) with 6 angular channels (two chunks of 3), one and two species
+        "tiny_K17_T1": lambda: wl.tiny_workload(11, n_species=1, sizes=(35, 6), box=(7.2, 4.1),
+                                                model=wl.ModelSpec(1, 3.3, 2.9, 3, 5, 16, 16, 4, 2, 1, 6)),
+        "tiny_K17_T2": lambda: wl.tiny_workload(12, n_species=2, sizes=(12, 38), box=(4.4, 7.4),
+                                                model=wl.ModelSpec(2, 3.3, 2.9, 2, 5, 12, 16, 4, 2, 1, 5)),
         "cfg1a": lambda: wl.make_config(1),
         "cfg1b": lambda: wl.make_config(1, n_struct=2, variant="1b"),
         "cfg2": lambda: wl.make_config(2, n_struct=6),
