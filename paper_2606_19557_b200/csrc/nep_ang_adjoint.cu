@@ -362,7 +362,7 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
 int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
 {
     const ModelDev& m = c->m;
-    const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
+    const int nch = pick_nch(c), kpad = pick_kpad(m.KA);
     NEP_DISPATCH_NCH_K(nch, kpad, {
         constexpr int NK = NCH * K;
         if (m.T == 1) {

@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_fwd(StepArgs a)
 int launch_ang_fwd(nep_ctx* c, const StepArgs& a)
 {
     const ModelDev& m = c->m;
-    const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
+    const int nch = pick_nch(c), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
         const size_t base = SWEEP2_SMEM_BYTES + cA_chunk_bytes<NCH, K>(m) + 4 * (size_t)(m.T * m.T * m.KR * ((m.nR + 3) & ~3));

@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
 int launch_ang_tangent(nep_ctx* c, const StepArgs& a)
 {
     const ModelDev& m = c->m;
-    const int nch = pick_nch(m.nA), kpad = pick_kpad(m.KA);
+    const int nch = pick_nch(c), kpad = pick_kpad(m.KA);
     const unsigned gx = (unsigned)((c->b.nbs * WARP + PAIR_TB - 1) / PAIR_TB);
     NEP_DISPATCH_NCH_K(nch, kpad, {
         const size_t base = SWEEP2_SMEM_BYTES + ((cA_chunk_bytes<NCH, K>(m) + 15) & ~(size_t)15);

@@ -577,8 +577,12 @@ void loss_args(nep_ctx* c, const StepArgs& a, LossArgs* o);
 void adam_args(nep_ctx* c, double lr, double b1, double b2, double eps, int variant, int64_t t, AdamArgs* o);
 
 // channels per thread for the angular sweeps: 3, 4 or 5 (fewer channels run as 3 with zero coefficients)
-inline int pick_nch(int nA)
+// A batch far below one resident wave of slices (config 1: 16 slices) is bound by the latency of a single warp's pair loop, and
+// blocks are free: such batches run 3 channels per thread (more channel chunks side by side, shorter contractions per pair).
+inline int pick_nch(const nep_ctx* c)
 {
+    const int nA = c->m.nA;
+    if (c->b.nbs > 0 && c->b.nbs < c->sm_count / 2) return 3;
     const int chunks = (nA + MAX_NCH - 1) / MAX_NCH;
     const int nch = (nA + chunks - 1) / chunks;
     return nch < 3 ? 3 : nch;
@@ -589,7 +593,7 @@ inline StepArgs make_args(nep_ctx* c)
 {
     StepArgs a;
     a.m = c->m; a.d = c->d; a.b = c->b; a.theta = c->theta; a.scaler = c->scaler; a.g = c->g;
-    const int nch = pick_nch(c->m.nA);
+    const int nch = pick_nch(c);
     a.nchunks = (c->m.nA + nch - 1) / nch;
     return a;
 }
