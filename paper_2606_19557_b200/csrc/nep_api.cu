@@ -184,6 +184,9 @@ int nep_destroy(nep_ctx* c)
     cudaStreamSynchronize(c->stream);
     graph_drop(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->side_stream) cudaStreamDestroy(c->side_stream);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     std::vector<void*> a = c->allocs;
     for (void* p : a) dev_free(c, p);
     if (c->h_stage) cudaFreeHost(c->h_stage);

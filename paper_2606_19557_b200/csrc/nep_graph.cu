@@ -29,9 +29,11 @@ static int capture_step(nep_ctx* c, double lr, double b1, double b2, double eps,
     const int64_t t_before = c->t_adam, launches_before = c->launches;
     const bool prof_paused = c->prof.paused;
     c->prof.paused = true;                                  // no event records inside a capture
+    c->capturing = true;
     int rc = launch_forward(c, false);
     if (!rc) rc = launch_loss_grad(c);
     if (!rc) rc = launch_adam(c, lr, b1, b2, eps, variant);
+    c->capturing = false;
     c->prof.paused = prof_paused;
     c->t_adam = t_before;                                   // capturing is not stepping
     c->graph_launches = (int)(c->launches - launches_before);

@@ -157,6 +157,8 @@ struct nep_ctx {
 
     // one training step as a CUDA graph (nep_graph.cu); graph_gen is bumped by every call that changes pointers or launch shapes
     cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr; cudaStream_t cap_stream = nullptr;
+    // small batches: the independent radial / angular sweeps of a step are captured as parallel branches (nep_misc.cu: SweepFork)
+    bool capturing = false; cudaStream_t side_stream = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     cudaGraphNode_t graph_loss_node = nullptr, graph_adam_node = nullptr;
     unsigned graph_loss_grid = 0, graph_adam_grid = 0;
     int64_t graph_gen = 0, graph_built_gen = -1, graph_seen_gen = -1;

@@ -247,6 +247,33 @@ int launch_gather_q(nep_ctx* c, float* dq)
 // ------------------------------------------------------------------------------------------------
 // the step: order of the sweeps
 // ------------------------------------------------------------------------------------------------
+// A batch far below one resident wave leaves most of the GPU idle and every kernel costs its launch-to-drain latency: while a step
+// is being captured into its graph, the radial sweep of a radial / angular pair (they are independent: both force sweeps add into F,
+// E_s, W_s with atomics; the tangent sweeps write different arrays) goes to a side stream and becomes a parallel branch of the graph.
+// At full size the pair gains nothing (the kernel launched first fills the GPU: profiles/r01d_summary.md), so it is not forked there.
+struct SweepFork {
+    nep_ctx* c; bool on; cudaStream_t main;
+    explicit SweepFork(nep_ctx* c_) : c(c_), on(false), main(c_->stream)
+    {
+        if (!c->capturing || c->b.nbs >= 2 * c->sm_count) return;
+        if (!c->side_stream && cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess) return;
+        if (!c->ev_fork && cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess) return;
+        if (!c->ev_join && cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) return;
+        if (cudaEventRecord(c->ev_fork, main) != cudaSuccess || cudaStreamWaitEvent(c->side_stream, c->ev_fork, 0) != cudaSuccess) return;
+        on = true;
+        c->stream = c->side_stream;          // the next launcher enqueues on the side stream
+    }
+    void back() { c->stream = main; }        // ... the one after it on the main stream again
+    int join()
+    {
+        c->stream = main;
+        if (!on) return NEP_OK;
+        NEP_CUDA(c, cudaEventRecord(c->ev_join, c->side_stream));
+        NEP_CUDA(c, cudaStreamWaitEvent(main, c->ev_join, 0));
+        return NEP_OK;
+    }
+};
+
 int launch_forward(nep_ctx* c, bool descriptors_only)
 {
     if (c->b.nbs == 0) return NEP_OK;
@@ -255,9 +282,12 @@ int launch_forward(nep_ctx* c, bool descriptors_only)
     if ((rc = launch_ang_fwd(c, a))) return rc;        // S1 + S2 (also clears E_s, W_s of the batch)
     if (descriptors_only) return NEP_OK;
     if ((rc = launch_ann_fwd(c, a))) return rc;        // S3
-    if ((rc = launch_rad_force(c, a))) return rc;      // S5 radial + S4
-    if ((rc = launch_ang_force(c, a))) return rc;      // S5 angular
-    return NEP_OK;
+    SweepFork f(c);
+    rc = launch_rad_force(c, a);                       // S5 radial + S4
+    f.back();
+    if (!rc) rc = launch_ang_force(c, a);              // S5 angular
+    const int rj = f.join();
+    return rc ? rc : rj;
 }
 
 int launch_loss_grad(nep_ctx* c)
@@ -266,8 +296,14 @@ int launch_loss_grad(nep_ctx* c)
     int rc;
     if ((rc = launch_loss(c, a))) return rc;           // S6 (clears g)
     if (c->b.nbs == 0) return NEP_OK;
-    if ((rc = launch_rad_tangent(c, a))) return rc;    // S7 radial
-    if ((rc = launch_ang_tangent(c, a))) return rc;    // S7 angular
+    {
+        SweepFork f(c);
+        rc = launch_rad_tangent(c, a);                 // S7 radial
+        f.back();
+        if (!rc) rc = launch_ang_tangent(c, a);        // S7 angular
+        const int rj = f.join();
+        if (rc || rj) return rc ? rc : rj;
+    }
     if ((rc = launch_ann_bwd(c, a))) return rc;        // S8
     if ((rc = launch_ang_adjoint(c, a))) return rc;    // S9
     return NEP_OK;
