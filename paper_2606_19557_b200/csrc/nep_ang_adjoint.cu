@@ -365,7 +365,9 @@ int launch_ang_adjoint(nep_ctx* c, const StepArgs& a)
     const int nch = pick_nch(c), kpad = pick_kpad(m.KA);
     NEP_DISPATCH_NCH_K(nch, kpad, {
         constexpr int NK = NCH * K;
-        if (m.T == 1) {
+        // one species: both passes in one block; a batch far below one resident wave is bound by the latency of one warp, and runs the
+        // two passes side by side as separate one-warp blocks (the multi-species kernel, whose table is then empty)
+        if (m.T == 1 && c->b.nbs >= c->sm_count / 2) {
             const int nw = PAIR_TB / WARP;
             const size_t base = (size_t)PAIR_TB * 64 + 4 * (size_t)nw * ((NK + 3) & ~3);
             const size_t smem = base + 4 * nw * staged_warp_floats(m, NCH) + STAGED_BAR_BYTES;
