@@ -349,11 +349,7 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
             const int tj = r / NKP, e = r - tj * NKP, n = e / K, k = e - n * K;
             if (!(e < NK && k < m.KA && n0 + n < m.nA)) continue;
             const float v = cs[r] - (tj > 0 ? cs[r - NKP] : 0.0f);
-#ifdef ADJ_NO_ATOMIC
-            if (v == 123.456f) a.g[0] = v;
-#else
             if (v != 0.0f) atomicAdd(a.g + m.o_cA + ((size_t)tj * m.nA + n0 + n) * m.KA + k + ti * tstep, v);
-#endif
         }
         __syncwarp();
     }

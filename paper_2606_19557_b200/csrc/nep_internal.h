@@ -98,7 +98,7 @@ struct BatchDev {
     float* eps;    // [Sb]       dL/dE_s
     float* G;      // [Sb][9]    dL/dW_s
     double* lacc;  // loss4 = {L, dE, dF, dV} at [4..7]; [8 + 4 b ..]: partial sums (dE)^2, |dF|^2, (dW)^2, sum eps N of block b of the loss kernel
-    unsigned* counter;   // [64] [0]: block ticket of the loss kernel; [8 + 4 k ..]: work queue of persistent sweep k (next, done)
+    unsigned* counter;   // [64] [0]: block ticket of the loss kernel
 };
 
 struct Profiler {

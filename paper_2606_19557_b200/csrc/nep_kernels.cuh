@@ -52,28 +52,7 @@ __device__ __forceinline__ void lane_init_slice(const StepArgs& a, Lane& L, int 
     L.ti = __ldg(a.d.type_p + (size_t)L.ds * WARP + L.lane);
 }
 
-// ------------------------------------------------------------------------------------------------
-// Persistent sweeps: a resident wave of warps takes work units (slices, or slice x pass) from a queue in global memory
-// (queue[0] = next unit, queue[1] = blocks that have finished; the last block to finish re-arms both: kernels of one stream
-// do not overlap).  The unit after the current one is fetched early, and the per-atom rows it will load in its prologue are
-// requested into L2 (cp.async.bulk.prefetch.L2, one instruction per contiguous block of rows) while the pairs of the current
-// unit are processed: the prologue then waits for L2 hits instead of DRAM.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned wq_issue(unsigned* queue)   // lane 0 takes a ticket; the value is valid after wq_value
-{
-    unsigned u = 0u;
-    if ((threadIdx.x & 31) == 0) u = atomicAdd(queue, 1u);
-    return u;
-}
-__device__ __forceinline__ unsigned wq_value(unsigned ticket) { return __shfl_sync(0xffffffffu, ticket, 0); }
-__device__ __forceinline__ void wq_finish(unsigned* queue)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        if (atomicAdd(queue + 1, 1u) == gridDim.x * gridDim.y * gridDim.z - 1u) { queue[0] = 0u; queue[1] = 0u; __threadfence(); }
-    }
-}
+// requests a block of global memory into L2 (one instruction per contiguous block)
 __device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes)   // bytes: a multiple of 16
 {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(p), "r"(bytes) : "memory");
@@ -158,7 +137,6 @@ __device__ __forceinline__ PairGeo pair_geo(const float4& rec)
 // latency of slot s+1, s+2 is covered by the arithmetic of slot s.  Each lane reads back only what it copied
 // itself, so cp.async.wait_group is the only synchronisation needed.
 constexpr int SWEEP_STAGES = 2;
-constexpr int SWEEP_SMEM_BYTES = PAIR_TB * 16 * SWEEP_STAGES;   // per block, at the start of dynamic shared memory
 
 __device__ __forceinline__ void cp_async16(float4* smem_dst, const float4* gsrc)
 {
@@ -168,34 +146,7 @@ __device__ __forceinline__ void cp_async16(float4* smem_dst, const float4* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
-// stage: this thread's first staging cell, cells of successive stages are PAIR_TB apart.
-// pre(active, record) runs converged on every lane of the warp for every slot (votes are allowed in it);
-// body(record) runs on the lanes that still have a record in this slot.
-template <class Pre, class Body>
-__device__ __forceinline__ void sweep_pairs(const float4* __restrict__ rec, int width, int cnt, float4* stage, Pre&& pre, Body&& body)
-{
-#pragma unroll
-    for (int st = 0; st < SWEEP_STAGES; ++st) {
-        if (st < width) cp_async16(stage + st * PAIR_TB, rec + (size_t)st * WARP);
-        cp_async_commit();
-    }
-    for (int s = 0; s < width; ++s) {
-        cp_async_wait<SWEEP_STAGES - 1>();
-        float4* cell = stage + (s % SWEEP_STAGES) * PAIR_TB;
-        const float4 cur = *cell;
-        if (s + SWEEP_STAGES < width) cp_async16(cell, rec + (size_t)(s + SWEEP_STAGES) * WARP);
-        cp_async_commit();
-        pre(s < cnt, cur);
-        if (s < cnt) body(cur);
-    }
-    cp_async_wait<0>();
-}
-template <class Body>
-__device__ __forceinline__ void sweep_pairs(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body&& body)
-{
-    sweep_pairs(rec, width, cnt, stage, [](bool, const float4&) {}, body);
-}
-// the same pipeline for a block of TB threads (staging cells of successive stages are TB apart)
+// one record per iteration: body(record) for the slots the lane has; staging cells of successive stages are TB apart
 template <int TB, class Body>
 __device__ __forceinline__ void sweep_pairs_tb(const float4* __restrict__ rec, int width, int cnt, float4* stage, Body&& body)
 {
@@ -371,14 +322,6 @@ __device__ __forceinline__ int ang_row(const ModelDev& m, int slot, int n)
 {
     const int a = slot < 4 ? slot : (slot == 4 ? m.l3 : m.l3 + m.has4);   // callers use a 3-body slot only if slot < l3
     return m.nR + a * m.nA + n;
-}
-// c[slot] = arr[row(slot, n)] for the invariants present, 0 otherwise  (arr: slice-blocked [D] rows, pointer at row 0)
-__device__ __forceinline__ void load_inv_coef(const ModelDev& m, const float* __restrict__ arr, int n, float* c)
-{
-#pragma unroll
-    for (int s = 0; s < 4; ++s) c[s] = s < m.l3 ? arr[(size_t)ang_row(m, s, n) * WARP] : 0.0f;
-    c[4] = m.has4 ? arr[(size_t)ang_row(m, 4, n) * WARP] : 0.0f;
-    c[5] = m.has5 ? arr[(size_t)ang_row(m, 5, n) * WARP] : 0.0f;
 }
 __device__ __forceinline__ void store_inv(const ModelDev& m, float* __restrict__ arr, int n, const float* q)
 {

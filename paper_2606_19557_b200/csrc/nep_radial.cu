@@ -11,27 +11,6 @@ namespace nep {
 
 constexpr int RAD_TB = 128;
 
-template <class Pre, class Body>
-__device__ __forceinline__ void sweep_pairs_rad(const float4* __restrict__ rec, int width, int cnt, float4* stage, Pre&& pre, Body&& body)
-{
-    // same pipeline as sweep_pairs with this file's block size
-#pragma unroll
-    for (int st = 0; st < SWEEP_STAGES; ++st) {
-        if (st < width) cp_async16(stage + st * RAD_TB, rec + (size_t)st * WARP);
-        cp_async_commit();
-    }
-    for (int s = 0; s < width; ++s) {
-        cp_async_wait<SWEEP_STAGES - 1>();
-        float4* cell = stage + (s % SWEEP_STAGES) * RAD_TB;
-        const float4 cur = *cell;
-        if (s + SWEEP_STAGES < width) cp_async16(cell, rec + (size_t)(s + SWEEP_STAGES) * WARP);
-        cp_async_commit();
-        pre(s < cnt, cur);
-        if (s < cnt) body(cur);
-    }
-    cp_async_wait<0>();
-}
-
 template <int K>
 __global__ void __launch_bounds__(RAD_TB) k_rad_force(StepArgs a)
 {
