@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                 Prep P;
                 P.p = pair_geo(rc4);
                 P.fv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, false>(P.p.r, rcinv, [&](int k, float fk, float) { P.fv[k] = fk; }, on);
+                cheb_basis<K, false, true>(P.p.r, rcinv, [&](int k, float fk, float) { P.fv[k] = fk; }, on);
                 return P;
             };
             auto contract = [&](const Prep& P) {
@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
                 P.p = pair_geo(rc4);
                 P.T = pair_tangent(ub, bbase, P.p, uix, uiy, uiz, G);
                 P.fv[2 * KH - 1] = 0.0f; P.dfv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, true>(P.p.r, rcinv, [&](int k, float fk, float dfk) { P.fv[k] = fk; P.dfv[k] = dfk; }, on);
+                cheb_basis<K, true, true>(P.p.r, rcinv, [&](int k, float fk, float dfk) { P.fv[k] = fk; P.dfv[k] = dfk; }, on);
                 return P;
             };
             auto contract = [&](const Prep& P) {
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
                 }
                 float fv[2 * KH];
                 fv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, false>(p.r, rcinv, [&](int k, float fk, float) { fv[k] = fk; });
+                cheb_basis<K, false, true>(p.r, rcinv, [&](int k, float fk, float) { fv[k] = fk; });
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) {
                     const float2 aa = dup2(al[n]);
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
                 }
                 float fv[2 * KH], dfv[2 * KH];
                 fv[2 * KH - 1] = 0.0f; dfv[2 * KH - 1] = 0.0f;
-                cheb_basis<K, true>(p.r, rcinv, [&](int k, float fk, float dfk) { fv[k] = fk; dfv[k] = dfk; });
+                cheb_basis<K, true, true>(p.r, rcinv, [&](int k, float fk, float dfk) { fv[k] = fk; dfv[k] = dfk; });
 #pragma unroll
                 for (int n = 0; n < NCH; ++n) {
                     const float2 dd = dup2(de[n]), bb = dup2(be[n]);

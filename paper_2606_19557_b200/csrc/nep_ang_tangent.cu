@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_tangent(StepArgs a)
         P.p = pair_geo(rc4);
         P.T = pair_tangent(ub, bbase, P.p, uix, uiy, uiz, G);
         float dg[NCH];
-        radial_gn<NCH, K, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, dg, on);
+        radial_gn<NCH, K, true, true>(P.p.r, rcinv, cbase + P.p.tj * CST, P.g, dg, on);
 #pragma unroll
         for (int n = 0; n < NCH; ++n) P.c[n] = dg[n] * P.T.t;
         return P;

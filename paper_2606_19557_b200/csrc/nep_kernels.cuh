@@ -301,12 +301,12 @@ __device__ __forceinline__ void coef_k(const float* __restrict__ cp, int k, floa
 }
 
 // g_n(r) = sum_k c_nk f_k(r) (and g_n') for the chunk's channels  (Eq. 16)
-template <int NCH, int K, bool DERIV>
+template <int NCH, int K, bool DERIV, bool FAST = false>
 __device__ __forceinline__ void radial_gn(float r, float rcinv, const float* __restrict__ cp, float* g, float* dg, float scale = 1.0f)
 {
 #pragma unroll
     for (int n = 0; n < NCH; ++n) { g[n] = 0.0f; if (DERIV) dg[n] = 0.0f; }
-    cheb_basis<K, DERIV>(r, rcinv, [&](int k, float fk, float dfk) {
+    cheb_basis<K, DERIV, FAST>(r, rcinv, [&](int k, float fk, float dfk) {
         float c[NCH];
         coef_k<NCH>(cp, k, c);
 #pragma unroll

@@ -56,13 +56,22 @@ __device__ __forceinline__ void sincospi_unit(float u, float& sn, float& cs)
 // constant (models with fewer functions run the next larger instantiation with zero-padded coefficients).
 // Without DERIV the derivative argument is 0 and its arithmetic is not generated.
 // ------------------------------------------------------------------------------------------------
+// The same from the special-function unit (sin.approx / cos.approx, absolute error ~1e-6): used by the sweeps of the second-order
+// path, whose results enter only the parameter gradient (tolerance 1e-3 relative); 4 instructions instead of 15.
+__device__ __forceinline__ void sincospi_unit_fast(float u, float& sn, float& cs)
+{
+    const float x = PI_F * (u - 0.5f);
+    cs = -__sinf(x);
+    sn = __cosf(x);
+}
+
 // scale multiplies every f_k and f_k' (they are linear in the three cutoff factors): a sweep masks a padded pair slot with scale = 0.
-template <int K, bool DERIV, class Body>
+template <int K, bool DERIV, bool FAST = false, class Body>
 __device__ __forceinline__ void cheb_basis(float r, float rcinv, Body&& body, float scale = 1.0f)
 {
     const float u = r * rcinv;
     float sn, cs;
-    sincospi_unit(u, sn, cs);
+    if (FAST) sincospi_unit_fast(u, sn, cs); else sincospi_unit(u, sn, cs);
     const float hfc = fmaf(0.25f, cs, 0.25f) * scale;      // 1/2 f_c
     const float um1 = u - 1.0f;
     const float x = fmaf(2.0f * um1, um1, -1.0f);

@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(RAD_TB) k_rad_tangent(StepArgs a)
             cur = p.tj;
         }
         const Tangent T = pair_tangent(ub, bbase, p, uix, uiy, uiz, G);
-        cheb_basis<K, true>(p.r, rcinv, [&](int k, float, float dfk) { bd[k] = fmaf(dfk, T.t, bd[k]); });
+        cheb_basis<K, true, true>(p.r, rcinv, [&](int k, float, float dfk) { bd[k] = fmaf(dfk, T.t, bd[k]); });
     };
     sweep_pairs2<RAD_TB>(sw.rec, sw.width, sw.cnt, stage_s + threadIdx.x, [&](const float4& ra, const float4& rb, bool has2) {
         one(ra);
