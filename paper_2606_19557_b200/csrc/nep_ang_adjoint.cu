@@ -154,15 +154,19 @@ __global__ void __launch_bounds__(PAIR_TB) k_ang_adjoint(StepArgs a)
             });
         }
         // every lane targets the same block of coefficients: reduce-scatter over the lanes, then shared-memory adds into the block's table
-        constexpr int P = NK <= 32 ? 32 : (NK <= 64 ? 64 : 128), PL = P / 32;
-        float v[P];
-#pragma unroll
-        for (int e = 0; e < P; ++e) v[e] = e < NK ? accv(e / K, e % K) : 0.0f;
-        warp_reduce_scatter<P>(v);
+        // (at most 64 values at a time: a larger register array would go to local memory)
+        constexpr int P = NK <= 32 ? 32 : 64, PL = P / 32;
         const int lane = threadIdx.x & 31;
 #pragma unroll
-        for (int j = 0; j < PL; ++j)
-            if (PL * lane + j < NK) atomicAdd(tab_all + PL * lane + j, v[j]);
+        for (int base = 0; base < NK; base += P) {
+            float v[P];
+#pragma unroll
+            for (int e = 0; e < P; ++e) v[e] = base + e < NK ? accv((base + e) / K, (base + e) % K) : 0.0f;
+            warp_reduce_scatter<P>(v);
+#pragma unroll
+            for (int j = 0; j < PL; ++j)
+                if (base + PL * lane + j < NK) atomicAdd(tab_all + base + PL * lane + j, v[j]);
+        }
     }
     // no block barrier: a warp leaves when it is done; the last one of the block (ticket) adds the table to g
     __syncwarp();
@@ -319,7 +323,7 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
     // shared memory per warp at five species, 8 instead of 6 warps per SM).
     const int nquad = (TR * NKP) >> 2;
     float* cs = tab + (size_t)WARP * LS;                 // [T * NKP] column sums of the current centre type
-    constexpr int P = NK <= 32 ? 32 : (NK <= 64 ? 64 : 128), PL = P / 32;
+    constexpr int P = NK <= 32 ? 32 : 64, PL = P / 32;   // at most 64 values at a time (a larger register array would go to local memory)
     const size_t tstep = (size_t)T * m.nA * m.KA;
     for (int ti = 0; ti < T; ++ti) {
         const unsigned bm = __ballot_sync(0xffffffffu, L.ti == ti);
@@ -336,13 +340,16 @@ __global__ void __launch_bounds__(WARP) k_ang_adjoint_ms(StepArgs a, int ahead)
         }
         {
             const bool in = lane >= c0 && lane < c1;
-            float v[P];
 #pragma unroll
-            for (int e = 0; e < P; ++e) v[e] = in ? accv(e) : 0.0f;
-            warp_reduce_scatter<P>(v);
+            for (int base = 0; base < NKP; base += P) {
+                float v[P];
 #pragma unroll
-            for (int j = 0; j < PL; ++j)
-                if (PL * lane + j < NKP) cs[TR * NKP + PL * lane + j] = v[j];
+                for (int e = 0; e < P; ++e) v[e] = in ? accv(base + e) : 0.0f;
+                warp_reduce_scatter<P>(v);
+#pragma unroll
+                for (int j = 0; j < PL; ++j)
+                    if (base + PL * lane + j < NKP) cs[TR * NKP + base + PL * lane + j] = v[j];
+            }
         }
         __syncwarp();
         for (int r = lane; r < T * NKP; r += WARP) {
