@@ -144,6 +144,28 @@ int nep_get_scaler(nep_ctx* ctx, double* s);
 int nep_compute_descriptor_range(nep_ctx* ctx, double* qmin, double* qmax);
 int nep_set_scaler_from_range(nep_ctx* ctx, const double* qmin, const double* qmax);
 
+/* Eq. 2 without a context and without an allocator: s_v = 1 / (max_i q_v^i - min_i q_v^i) for v = 0..n_desc-1 over
+ * the n_atoms rows of a descriptor matrix that already sits on the device.  Who needs it: every other call here takes its device
+ * memory from the nep_alloc_fn a context was created with, so a caller that has no allocator to lend -- its framework's pool owns
+ * the whole GPU and a raw cudaMalloc would fail, it is in the middle of stream-ordered work that cudaMalloc's device-wide
+ * synchronisation would stall, or it is plain C / Fortran holding two device pointers and nothing else -- cannot use
+ * nep_compute_scaler.  This call allocates nothing, on the device or through any library: its working memory is an array of
+ * NEP_STATIC_SCRATCH_BYTES that is part of the library image (each GPU that loads the library keeps it until the process ends).
+ *   q_dev  [n_atoms][n_desc] float, device, row-major, unscaled descriptors (the layout nep_get_descriptors returns);
+ *   s_dev  [n_desc] float, device, written by the kernel; a component without a range (all rows equal, or n_atoms == 0) gets 1,
+ *          by the same fp32 rule as nep_compute_scaler (DESIGN G10);
+ *   cuda_stream: a cudaStream_t (NULL = default stream) on the CURRENT device, which must also own q_dev and s_dev; the work is
+ *          enqueued there and the call returns without synchronising.  Both buffers stay the caller's.
+ * Limits and sharing: n_desc <= NEP_STATIC_MAX_DESCRIPTORS (NEP_ECAPACITY beyond, nothing launched); n_atoms is not limited.
+ * All calls on a device use the one array: calls whose kernels could run at the same time on that GPU (two streams, two
+ * threads) race and must be serialised by the caller; calls in stream order are fine, nothing has to be cleared in between.
+ * The first call on each device looks up the array's address and caches it: make it before, not during, a stream capture.
+ * Errors: NEP_EINVAL (n_desc < 1, n_atoms < 0, NULL pointer), NEP_ECAPACITY, NEP_ECUDA; the message is nep_last_error(NULL)
+ * (per host thread, shared with nep_create's). */
+#define NEP_STATIC_MAX_DESCRIPTORS 128
+#define NEP_STATIC_SCRATCH_BYTES 303360
+int nep_scaler_static(const float* q_dev, int64_t n_atoms, int n_desc, float* s_dev, void* cuda_stream);
+
 /* Mini-batch = a list of structure ids ("batch" of Table I).  ids == NULL: the whole set.
  * ids are copied to the device; the same id must not appear twice.  Selecting the batch that is already current (full-batch
  * training does so every step) uploads its tables again but keeps the tables derived from them on the device. */

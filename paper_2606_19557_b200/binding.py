@@ -50,6 +50,7 @@ SIGNATURES = {
     "nep_get_scaler": (C.c_int, [_P, _P]),
     "nep_compute_descriptor_range": (C.c_int, [_P, _P, _P]),
     "nep_set_scaler_from_range": (C.c_int, [_P, _P, _P]),
+    "nep_scaler_static": (C.c_int, [_P, C.c_int64, C.c_int, _P, _P]),
     "nep_set_batch": (C.c_int, [_P, C.c_int, _P]),
     "nep_forward": (C.c_int, [_P, _P, _P, _P, C.c_int]),
     "nep_get_descriptors": (C.c_int, [_P, _P]),
@@ -101,6 +102,28 @@ def _np(a, dtype, shape=None) -> np.ndarray:
 
 def _ptr(a: Optional[np.ndarray]):
     return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+NEP_STATIC_MAX_DESCRIPTORS = 128
+
+
+def scaler_static(q, s, stream=None) -> None:
+    """nep_scaler_static (include/nep.h): Eq. 2's scaler s [D] from the descriptor matrix q [N][D], both float32 CUDA tensors that
+    the CALLER owns, on the current device.  For callers that cannot give the library an allocator (a context needs one) and
+    cannot call cudaMalloc themselves: the call allocates nothing, its working memory is a fixed array inside the library, so
+    D <= NEP_STATIC_MAX_DESCRIPTORS (NepError NEP_ECAPACITY beyond) and calls that could overlap on one GPU must be serialised.
+    Enqueues on `stream` (default: torch's current stream) and returns without synchronising."""
+    import torch
+    L = load_library()
+    if not (q.is_cuda and s.is_cuda and q.dtype == torch.float32 and s.dtype == torch.float32 and q.is_contiguous() and s.is_contiguous()):
+        raise ValueError("q and s must be contiguous float32 CUDA tensors")
+    if q.dim() != 2 or s.numel() != q.shape[1]:
+        raise ValueError("q must be [N][D] and s [D]")
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    rc = L.nep_scaler_static(C.c_void_p(q.data_ptr()), int(q.shape[0]), int(q.shape[1]), C.c_void_p(s.data_ptr()), C.c_void_p(stream.cuda_stream))
+    if rc != NEP_OK:
+        raise NepError(rc, (L.nep_last_error(None) or b"").decode())
 
 
 class Nep:
