@@ -168,11 +168,39 @@ class DataParallelNep:
     def local_batch_shape(self):
         return self.nep.batch_shape()
 
-    def step(self, lam, lr: float, fetch_loss: bool = False):
+    def step(self, lam, lr: float, fetch_loss: bool = False, variant: int = 0):
         """One training step on the current batch: forward, loss + gradient, the all-reduce, Adam."""
         self.nep.forward_device()
         self.nep.loss_grad(lam[0], lam[1], lam[2], fetch_loss=False)
         g, l4 = self.nep.grad_loss_tensors()
         allreduce_grad_loss(g, l4, self.group, getattr(self.nep, "stream", None))
-        self.nep.adam_step(lr)
+        self.nep.adam_step(lr, variant=variant)
         return l4.cpu().numpy() if fetch_loss else None
+
+    # ---- the surface trainer.Trainer drives (P:99-103: mini-batches, two-stage schedule, plateau decay), with GLOBAL ids: every
+    #      rank runs the same Trainer with the same seed, so all of them select the same batches and see the same whole-batch loss
+    #      terms, hence the same learning-rate decisions -- no broadcast is needed ----
+    @property
+    def n_struct(self) -> int:
+        return len(self.n_atoms)
+
+    def train_step(self, lambda_E: float, lambda_F: float, lambda_V: float, lr: float, variant: int = 0):
+        self.step((lambda_E, lambda_F, lambda_V), lr, fetch_loss=False, variant=variant)
+
+    def get_loss(self) -> np.ndarray:
+        """{L, dE, dF, dV} of the WHOLE batch of the last step (summed over the ranks), on the host."""
+        return self.nep.grad_loss_tensors()[1].cpu().numpy().copy()
+
+    def batch_counts(self):
+        """(S_b, N_b, S_v) of the whole current batch (the counts Eqs. 5-7 were divided by)."""
+        return self._whole
+
+    def forward_device(self):
+        self.nep.forward_device()
+
+    def loss_grad(self, lambda_E: float, lambda_F: float, lambda_V: float, fetch_loss: bool = True):
+        """Loss terms and gradient of the whole batch (all-reduced); the RMSE report of Trainer.rmse goes through here."""
+        self.nep.loss_grad(lambda_E, lambda_F, lambda_V, fetch_loss=False)
+        g, l4 = self.nep.grad_loss_tensors()
+        allreduce_grad_loss(g, l4, self.group, getattr(self.nep, "stream", None))
+        return l4.cpu().numpy().copy() if fetch_loss else None

@@ -105,6 +105,72 @@ def _rank_dp_nep(rank, world, port, out):
         dist.destroy_process_group()
 
 
+def _rank_trainer(rank, world, port, out):
+    import torch.distributed as dist
+    from paper_2606_19557_b200 import trainer as T
+    from tests._oracle_nep import OracleNep
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        O.set_num_threads(1)
+        w, prob, hv, cfg = _trainer_problem()
+        d = dp.DataParallelNep(w.model, w.structures, rank, world, nep_factory=OracleNep.from_model)
+        d.load(prob.E, prob.F, prob.W, hv)
+        d.nep.set_params(prob.theta); d.nep.set_scaler(prob.scaler)
+        tr = T.Trainer(d, cfg)
+        hist = tr.fit()
+        r = tr.rmse(chunk=4)
+        out.put((rank, d.nep.get_params(), [(h.lr, h.loss, h.dE, h.dF, h.dV) for h in hist], r))
+    finally:
+        dist.destroy_process_group()
+
+
+def _trainer_problem():
+    from paper_2606_19557_b200 import trainer as T
+    w = wl.tiny_workload(11, n_species=2, sizes=(5, 9, 3, 7, 6, 4), box=(3.4, 4.3, 3.1, 3.9, 3.6, 4.0))
+    prob = H.make_problem(w)
+    hv = np.array([1, 0, 1, 1, 1, 0], np.uint8)
+    cfg = T.TrainConfig(epoch=3, batch=4, stage1=T.StageSpec(5e-3, 1.0, 2.0, 0.5), stage2=T.StageSpec(2e-3, 2.0, 1.0, 1.0),
+                        start_stage2=2, scheduler_patience=0, scheduler_factor=0.5, seed=3)
+    return w, prob, hv, cfg
+
+
+def test_trainer_over_two_ranks_follows_the_one_rank_trajectory_gloo_world2():
+    """P:99-103 data-parallel: the same Trainer (same seed) on two ranks, each holding its share of the structures, selects the same
+    global mini-batches, sees the whole batch's loss terms after the all-reduce, takes the same learning-rate decisions, and lands on
+    the parameters, the epoch records and the RMSE report of one context holding everything."""
+    import torch.multiprocessing as mp
+    from paper_2606_19557_b200 import trainer as T
+    from tests._oracle_nep import OracleNep
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rank_trainer, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted((out.get(timeout=300) for _ in range(2)), key=lambda r: r[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    w, prob, hv, cfg = _trainer_problem()
+    one = OracleNep(w.model)
+    one.load_structure_set(w.structures, prob.E, prob.F, prob.W, hv)
+    one.build_neighbors()
+    one.set_params(prob.theta); one.set_scaler(prob.scaler)
+    tr = T.Trainer(one, cfg)
+    hist = tr.fit()
+    r_one = tr.rmse(chunk=4)
+    ref = [(h.lr, h.loss, h.dE, h.dF, h.dV) for h in hist]
+    assert len(ref) == 3 and len({h[0] for h in ref}) > 1                      # the rate changed along the way (stage 2 / decay)
+    moved = np.linalg.norm(one.get_params().astype(np.float64) - prob.theta)
+    for _, th, h, r in res:
+        assert np.linalg.norm(th.astype(np.float64) - one.get_params()) <= 1e-4 * moved
+        assert [x[0] for x in h] == [x[0] for x in ref]                        # identical learning-rate sequence
+        assert np.allclose(np.array(h)[:, 1:], np.array(ref)[:, 1:], rtol=1e-5)
+        for k in r_one:
+            assert r[k] == pytest.approx(r_one[k], rel=1e-5)
+
+
 def test_dataparallel_nep_scaler_and_step_gloo_world2():
     """Eq. 2 is over every atom of the set: two ranks with different structures (and different local ranges) must end with
     the identical scaler, equal to the oracle's over the union; one DataParallelNep.step then lands both on the parameters
