@@ -207,8 +207,9 @@ int nep_adam_step(nep_ctx* ctx, double lr, double beta1, double beta2, double ep
 /* One training step = nep_forward + nep_loss_grad + nep_adam_step on the current batch, without outputs (the loss terms stay
  * on the device: nep_get_loss).  use_graph != 0: the step's kernels are captured once into a CUDA graph and replayed with one
  * launch; loss weights, learning rate and the bias corrections of Eq. 11 are written into the graph's nodes before each
- * replay, so they may change from step to step.  nep_set_batch, nep_set_batch_normalisers, nep_set_labels and
- * nep_load_structures invalidate the graph (nep_set_batch only if the batch's shape changes); the first step after that runs as
+ * replay, so they may change from step to step.  nep_set_batch, nep_set_batch_normalisers, nep_set_labels,
+ * nep_load_structures and nep_build_neighbors invalidate the graph (nep_set_batch only if the batch's shape or its number of atoms
+ * per species changes); the first step after that runs as
  * the three calls, the graph is captured when the same batch is stepped a second time.  Same results as the three calls. */
 int nep_train_step(nep_ctx* ctx, double lambda_E, double lambda_F, double lambda_V, double lr, double beta1, double beta2,
                    double eps, int variant, int use_graph);
@@ -227,6 +228,16 @@ int nep_profile_enable(nep_ctx* ctx, int on);
  * of its steps only, so that the event records do not sit between the kernels of every step. */
 int nep_profile_pause(nep_ctx* ctx, int paused);
 int nep_profile_read(nep_ctx* ctx, int cap, const char** names, double* ms, int64_t* launches, int* n);
+
+/* 1 if the network kernels of this context (S3, S8) run as tcgen05 tiles, 0 if the model's tiles do not fit in shared memory /
+ * tensor memory (or NEP_ANN_FFMA=1 was set when the context was created) and the FFMA tiles are used.  Tests use it to make sure a
+ * parity case really exercises the tensor-core path. */
+int nep_network_on_tensor_cores(const nep_ctx* ctx);
+
+/* Measurement aid, no context: runs a register-resident FP32 FMA loop (32 independent chains per thread, 2048 threads per SM)
+ * on the current device for a few milliseconds and returns the rate it reached in TFLOP/s (2 flops per FMA) -- the measured
+ * counterpart of the derived FP32 peak bench.py's "alu" roofline divides by.  Synchronises cuda_stream. */
+int nep_measure_fp32_peak(void* cuda_stream, double* tflops);
 
 /* Sizes of the loaded set / current batch: {S, N, P_R, P_A, S_b, N_b, P_R_b, P_A_b}. */
 int nep_get_sizes(nep_ctx* ctx, int64_t* sizes8);

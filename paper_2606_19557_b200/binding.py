@@ -65,6 +65,8 @@ SIGNATURES = {
     "nep_profile_enable": (C.c_int, [_P, C.c_int]),
     "nep_profile_pause": (C.c_int, [_P, C.c_int]),
     "nep_profile_read": (C.c_int, [_P, C.c_int, _P, _P, _P, C.POINTER(C.c_int)]),
+    "nep_network_on_tensor_cores": (C.c_int, [_P]),
+    "nep_measure_fp32_peak": (C.c_int, [_P, C.POINTER(C.c_double)]),
     "nep_get_sizes": (C.c_int, [_P, _P]),
 }
 
@@ -124,6 +126,19 @@ def scaler_static(q, s, stream=None) -> None:
     rc = L.nep_scaler_static(C.c_void_p(q.data_ptr()), int(q.shape[0]), int(q.shape[1]), C.c_void_p(s.data_ptr()), C.c_void_p(stream.cuda_stream))
     if rc != NEP_OK:
         raise NepError(rc, (L.nep_last_error(None) or b"").decode())
+
+
+def measure_fp32_peak(stream=None) -> float:
+    """nep_measure_fp32_peak: TFLOP/s of a register-resident FP32 FMA loop on the current device (measurement aid for bench.py)."""
+    import torch
+    L = load_library()
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    v = C.c_double(0.0)
+    rc = L.nep_measure_fp32_peak(C.c_void_p(stream.cuda_stream), C.byref(v))
+    if rc != NEP_OK:
+        raise NepError(rc, (L.nep_last_error(None) or b"").decode())
+    return v.value
 
 
 class Nep:
@@ -275,6 +290,7 @@ class Nep:
                                              _ptr(W), _ptr(hv)))
         self.n_struct, self.n_atoms_total = S, N
         self._n_atoms = n_atoms.copy()
+        self._has_virial = np.ones(S, np.uint8) if hv is None else hv.copy()     # the mask the context normalises Eq. 7 with
 
     def load_structure_set(self, st, E=None, F=None, W=None, has_virial=None):
         self.load_structures(st.n_atoms, st.pos, st.box, st.type, E, F, W, has_virial)
@@ -284,6 +300,7 @@ class Nep:
         E = _np(E, np.float64, (S,)); F = _np(F, np.float64, (N, 3)); W = _np(W, np.float64, (S, 9))
         hv = None if has_virial is None else _np(has_virial, np.uint8, (S,))
         self._ck(self._L.nep_set_labels(self._h, _ptr(E), _ptr(F), _ptr(W), _ptr(hv)))
+        self._has_virial = np.ones(S, np.uint8) if hv is None else hv.copy()
 
     def build_neighbors(self):
         self._ck(self._L.nep_build_neighbors(self._h))
@@ -367,6 +384,13 @@ class Nep:
         ids = self._batch_ids
         return len(ids), int(self._n_atoms[ids].sum()) if len(ids) else 0
 
+    def batch_counts(self):
+        """(S_b, N_b, S_v) of the current batch: the counts Eqs. 5-7 divide by (S_v = structures whose virial label counts, from the
+        mask given with the labels)."""
+        ids = self._batch_ids
+        Sb, Nb = self.batch_shape()
+        return Sb, Nb, int(self._has_virial[ids].sum()) if len(ids) else 0
+
     def forward(self, want=("E", "F", "W")):
         """S1-S5.  Returns host float32 arrays (E [S_b], F [N_b,3], W [S_b,9]) (None for those not wanted)."""
         Sb, Nb = self.batch_shape()
@@ -447,6 +471,9 @@ class Nep:
         self._ck(self._L.nep_profile_read(self._h, cap, C.cast(names, C.c_void_p), C.cast(ms, C.c_void_p), C.cast(ln, C.c_void_p),
                                           C.byref(n)))
         return {names[i].decode(): (ms[i], ln[i]) for i in range(n.value)}
+
+    def network_on_tensor_cores(self) -> bool:
+        return bool(self._L.nep_network_on_tensor_cores(self._h))
 
     def get_sizes(self) -> dict:
         s = np.zeros(8, np.int64)

@@ -79,6 +79,7 @@ namespace nep {
 int upload_slot_tables(nep_ctx* c)
 {
     c->batch_tables_valid = false;     // the type-sorted atom list of a batch depends on the slot order
+    ++c->graph_gen;                    // the tables move to new buffers: a captured step graph points at the old ones
     DataDev& d = c->d;
     const int T = c->m.T;
     std::vector<int> type_p((size_t)c->NP, -1), rank_p((size_t)c->NP, 0), orig_p((size_t)c->NP, -1);
@@ -337,6 +338,8 @@ int nep_build_neighbors(nep_ctx* c)
     CHECK_CTX(c);
     if (!c->have_data) return fail(c, NEP_ESTATE, "nep_build_neighbors before nep_load_structures");
     c->batch_tables_valid = false;
+    ++c->graph_gen;                            // the lists, the pair cache and the slot tables are released and allocated again: a captured
+                                               // step graph holds the old pointers (StepArgs.d by value) whatever the batch tables look like
     int rc = build_neighbors_dev(c);
     if (rc) return rc;
     c->have_nbrs = true;
@@ -663,12 +666,15 @@ int nep_set_batch(nep_ctx* c, int n, const int* ids)
         const int s = ids ? ids[k] : k;
         for (int t = 0; t < T; ++t) tot[t] += c->h_tcount[(size_t)s * T + t];
     }
+    // a batch of the same shape in the same buffers leaves a captured step graph valid.  The snapshot is taken BEFORE the first tile
+    // of each species is rewritten: StepArgs carries tile_start by value, so two batches that agree in every count but not in their
+    // composition (other atoms per species) need a new capture.
+    const BatchDev b_before = c->b;
     BatchDev& b = c->b;
     int ntiles = 0;
     for (int t = 0; t < T; ++t) { b.tile_start[t] = ntiles; ntiles += (int)((tot[t] + TM - 1) / TM); }
     for (int t = T; t <= MAX_T; ++t) b.tile_start[t] = ntiles;
     c->forward_valid = c->grad_valid = false;
-    const BatchDev b_before = c->b;            // a batch of the same shape in the same buffers leaves a captured step graph valid
     int rc = ensure_batch_capacity(c, std::max<int64_t>(nbs64 * WARP, WARP), std::max(Sb, 1), std::max(nbs, 1), std::max<int64_t>((int64_t)ntiles * TM, TM));
     if (rc) {   // no batch is selected after a failed allocation: the step calls launch nothing
         b.Sb = b.Sv = 0; b.Nb = 0; b.nbs = 0; b.NBP = 0; b.ntiles = 0;
@@ -876,6 +882,8 @@ int nep_profile_read(nep_ctx* c, int cap, const char** names, double* ms, int64_
     c->prof.acc.clear();
     return NEP_OK;
 }
+
+int nep_network_on_tensor_cores(const nep_ctx* c) { return c && c->ann_tc ? 1 : 0; }
 
 int nep_get_sizes(nep_ctx* c, int64_t* s)
 {

@@ -201,7 +201,11 @@ __global__ void __launch_bounds__(256) k_descriptor_range(StepArgs a, float* rng
     if (threadIdx.x == 0) { rng[v] = slo[0]; rng[a.m.DP + v] = shi[0]; }
 }
 // s = 1 / (max - min) (Eq. 2).  A component without a range gets s = 1 (reading G10): "without a range" is a range below
-// the resolution of the arithmetic that produced q, here fp32 sums: 64 eps_fp32 max(1, max |q|) (the fp64 oracle: 1e-12).
+// the resolution of the arithmetic that produced q, here fp32 sums: 64 eps_fp32 max(1e-4, max |q|).  The rule is relative to the
+// component's magnitude, so that a small but well resolved component (a 5-body invariant of a sparse structure, |q| ~ 1e-6) keeps
+// its 1 / range as in the fp64 oracle (whose floor is 1e-12).  It cannot be purely relative: a component that vanishes by symmetry
+// (l = 1, 3 moments of a centrosymmetric lattice) is the SQUARE of fp32 round-off, ~1e-12 with a range of the same size, and
+// 1 / range of that would be ~1e12; the absolute floor 64 eps 1e-4 = 7.6e-10 stays two orders above it.
 __global__ void k_scaler_from_range(int D, int DP, const float* __restrict__ rng, float* __restrict__ s)
 {
     const int v = blockIdx.x * blockDim.x + threadIdx.x;
@@ -210,7 +214,7 @@ __global__ void k_scaler_from_range(int D, int DP, const float* __restrict__ rng
     if (v < D) {
         const float lo = rng[v], hi = rng[DP + v];
         const float range = hi - lo, am = fmaxf(fabsf(lo), fabsf(hi));
-        out = (hi >= lo && isfinite(range) && range > 64.0f * 1.1920929e-7f * fmaxf(1.0f, am)) ? 1.0f / range : 1.0f;
+        out = (hi >= lo && isfinite(range) && range > 64.0f * 1.1920929e-7f * fmaxf(1e-4f, am)) ? 1.0f / range : 1.0f;
     }
     s[v] = out;
 }

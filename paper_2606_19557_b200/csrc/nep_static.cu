@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(STATIC_THREADS) k_scaler_static(const float* _
         for (unsigned b = 0; b < gridDim.x; ++b) { lo = fminf(lo, __ldcg(&sc->lo[b][tid])); hi = fmaxf(hi, __ldcg(&sc->hi[b][tid])); }
         // Eq. 2; a component without a range gets s = 1 -- the same rule, in the same arithmetic, as k_scaler_from_range
         const float range = hi - lo, am = fmaxf(fabsf(lo), fabsf(hi));
-        s[tid] = (hi >= lo && isfinite(range) && range > 64.0f * 1.1920929e-7f * fmaxf(1.0f, am)) ? 1.0f / range : 1.0f;
+        s[tid] = (hi >= lo && isfinite(range) && range > 64.0f * 1.1920929e-7f * fmaxf(1e-4f, am)) ? 1.0f / range : 1.0f;
     }
     if (tid == 0) sc->ticket = 0u;
 }

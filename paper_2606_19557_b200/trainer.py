@@ -133,22 +133,36 @@ class Trainer:
                 callback(rec)
         return self.history
 
-    def rmse(self, n_atoms: Sequence[int], has_virial: Optional[Sequence[int]] = None, chunk: int = 1024) -> dict:
+    def rmse(self, n_atoms: Optional[Sequence[int]] = None, has_virial: Optional[Sequence[int]] = None, chunk: int = 1024) -> dict:
         """Root-mean-square errors over the whole loaded set: energy and virial per atom, force per component.
 
         RMSE = sqrt(Delta) with the mean squares Delta_E, Delta_F, Delta_V of Eqs. 5-7 (P:69-73), which nep_loss_grad returns;
-        the set is evaluated in chunks of structures whose Deltas are recombined with their counts (S_b, N_b and the number
-        of structures with virial labels).  No arithmetic of Eqs. 5-7 is repeated here."""
+        the set is evaluated in chunks of structures whose Deltas are recombined with the counts they were divided by (S_b, N_b
+        and S_v, the number of structures with virial labels).  The counts come from the context (`batch_counts`), which knows
+        the virial mask its labels were loaded with; n_atoms / has_virial are only consulted for a context without
+        `batch_counts`, and a has_virial that contradicts the context's mask is an error rather than a silently wrong weight.
+        No arithmetic of Eqs. 5-7 is repeated here."""
         nep = self.nep
-        n_atoms = np.asarray(n_atoms, dtype=np.int64)
-        hv = np.ones(len(n_atoms), dtype=np.int64) if has_virial is None else np.asarray(has_virial, dtype=np.int64)
+        own = hasattr(nep, "batch_counts")
+        if not own:
+            if n_atoms is None:
+                raise ValueError("this context has no batch_counts(): pass n_atoms (and has_virial if the labels carry a mask)")
+            n_atoms = np.asarray(n_atoms, dtype=np.int64)
+            hv = np.ones(len(n_atoms), dtype=np.int64) if has_virial is None else np.asarray(has_virial, dtype=np.int64)
         wE = wF = wV = 0.0
+        S = N = Sv = 0
         for i in range(0, nep.n_struct, chunk):
             ids = np.arange(i, min(i + chunk, nep.n_struct), dtype=np.int32)
             nep.set_batch(ids)
+            if own:
+                sb, nb, sv = nep.batch_counts()
+                if has_virial is not None and sv != int(np.asarray(has_virial, dtype=np.int64)[ids].sum()):
+                    raise ValueError("has_virial differs from the mask the context's labels were loaded with")
+            else:
+                sb, nb, sv = len(ids), int(n_atoms[ids].sum()), int(hv[ids].sum())
             nep.forward_device()
             _, dE, dF, dV = nep.loss_grad(1.0, 1.0, 1.0, fetch_loss=True)
-            wE += dE * len(ids); wF += dF * int(n_atoms[ids].sum()); wV += dV * int(hv[ids].sum())
-        S, N, Sv = nep.n_struct, int(n_atoms.sum()), int(hv.sum())
+            wE += dE * sb; wF += dF * nb; wV += dV * sv
+            S += sb; N += nb; Sv += sv
         return {"energy_per_atom": (wE / max(S, 1)) ** 0.5, "force": (wF / max(N, 1)) ** 0.5,
                 "virial_per_atom": (wV / Sv) ** 0.5 if Sv else 0.0}

@@ -70,6 +70,11 @@ class OracleNep:
     def batch_shape(self):
         return len(self.batch), int(self.st.n_atoms[self.batch].sum()) if self.batch else 0
 
+    def batch_counts(self):
+        Sb, Nb = self.batch_shape()
+        hv = None if self.labels is None else self.labels[3]
+        return Sb, Nb, Sb if hv is None else int(np.asarray(hv)[self.batch].sum()) if self.batch else 0
+
     def set_batch_normalisers(self, S, N, Sv):
         self.whole = (S, N, Sv)
 

@@ -20,11 +20,12 @@ def _draw(model, data, seed):
     return pd.network((q * s).mean(axis=0)).copy(), s
 
 
-@pytest.mark.parametrize("cfg", [2, 3, 4, "5 smallest model", "5 largest model"])
+@pytest.mark.parametrize("cfg", [2, 3, 4, "5 smallest model", "5 largest model", "5 model 6"])
 def test_full_size_batch_against_oracle(cfg):
     from paper_2606_19557_b200.binding import Nep
     if isinstance(cfg, str):          # config 5: the two ends of the model-complexity sweep (n_max 4 / 8, basis 8 / 12, 30 / 100 neurons)
-        w = wl.make_config(5, model=wl.config5_sweep()[0 if "smallest" in cfg else -1])
+        # ... and model 6 (n_max 8, basis 12, 30 neurons: D = 63, 13 radial functions), the widest tile the tensor-core kernels run
+        w = wl.make_config(5, model=wl.config5_sweep()[0 if "smallest" in cfg else 6 if "model 6" in cfg else -1])
     else:
         w = wl.make_config(cfg)
     st = w.structures

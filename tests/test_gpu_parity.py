@@ -39,6 +39,23 @@ def _cases():
         "cfg5_small_model": lambda: wl.make_config(5, n_struct=8),
         "cfg5_large_model": lambda: wl.make_config(5, n_struct=8, model=m5[-1]),      # n_max 8, basis 12, 100 neurons
         "cfg5_mixed_model": lambda: wl.make_config(5, n_struct=6, model=m5[5]),       # n_max 8, basis 8, 100 neurons
+        # the other five models of config 5's sweep (index = 4 [n_max 8] + 2 [basis 12] + 1 [100 neurons]); models 4 and 6 have D = 63:
+        # eight K steps per tcgen05 product, accumulator width 112 / 128
+        "cfg5_model1": lambda: wl.make_config(5, n_struct=6, model=m5[1]),
+        "cfg5_model2": lambda: wl.make_config(5, n_struct=6, model=m5[2]),
+        "cfg5_model3": lambda: wl.make_config(5, n_struct=6, model=m5[3]),
+        "cfg5_model4": lambda: wl.make_config(5, n_struct=6, model=m5[4]),
+        "cfg5_model6": lambda: wl.make_config(5, n_struct=6, model=m5[6]),
+        # the widest network tiles that fit the tensor-core kernels, on ragged slices: D = 63 with three species; D = 125 (n_max 10 / 18:
+        # 19 angular channels) with 24 neurons; 128 neurons with D = 21; 100 neurons with two species (see TC_CASES below)
+        "tiny_D63_H40_T3": lambda: wl.tiny_workload(13, n_species=3, sizes=(33, 2, 40), box=(7.5, 3.1, 8.0),
+                                                    model=wl.ModelSpec(3, 3.2, 2.6, 8, 8, 4, 4, 4, 2, 1, 40)),
+        "tiny_D125_H24_T2": lambda: wl.tiny_workload(14, n_species=2, sizes=(35, 44), box=(7.2, 7.6),
+                                                     model=wl.ModelSpec(2, 3.3, 2.9, 10, 18, 4, 4, 4, 2, 1, 24)),
+        "tiny_D21_H128_T1": lambda: wl.tiny_workload(15, n_species=1, sizes=(37, 5), box=(7.3, 3.6),
+                                                     model=wl.ModelSpec(1, 3.2, 2.6, 2, 2, 4, 4, 4, 2, 1, 128)),
+        "tiny_D35_H100_T2": lambda: wl.tiny_workload(16, n_species=2, sizes=(6, 41), box=(3.9, 7.5),
+                                                     model=wl.ModelSpec(2, 3.2, 2.6, 4, 4, 8, 8, 4, 2, 1, 100)),
         "wide_T16": lambda: wl.tiny_workload(6, n_species=16, sizes=(40, 37), box=(7.0, 6.5),
                                              model=wl.ModelSpec(16, 3.2, 2.6, 3, 3, 4, 4, 4, 2, 1, 12)),
     }
@@ -46,6 +63,10 @@ def _cases():
 
 CASES = _cases()
 _cache = {}
+# cases whose network products must run on the tensor cores (nep_network_on_tensor_cores): a parity case that silently fell back
+# to the FFMA tiles would say nothing about the tcgen05 kernels
+TC_CASES = ["cfg2", "cfg3", "cfg4", "cfg5_small_model", "cfg5_model2", "cfg5_model4", "cfg5_model6", "tiny_D63_H40_T3", "tiny_D125_H24_T2",
+            "tiny_D21_H128_T1", "tiny_D35_H100_T2", "tiny_K17_T1"]
 
 
 def _prob(name):
@@ -61,6 +82,13 @@ def test_neighbor_lists_bit_exact(name):
         H.check_neighbors(nep, prob.data)
         s = nep.get_sizes()
         assert s["P_R"] == len(prob.data.jR) and s["P_A"] == len(prob.data.jA) and s["N"] == prob.data.n_atoms_total
+
+
+@pytest.mark.parametrize("name", TC_CASES)
+def test_case_runs_on_the_tensor_core_network_kernels(name):
+    from paper_2606_19557_b200.binding import Nep
+    with Nep.from_model(CASES[name]().model) as nep:
+        assert nep.network_on_tensor_cores(), name
 
 
 @pytest.mark.parametrize("name", list(CASES))
@@ -151,6 +179,53 @@ def test_same_batch_selected_again():
             nep.train_step(*lam, 1e-3, use_graph=False)
         th_b = nep.get_params()
         assert np.linalg.norm(th_a - th_b) <= 1e-3 * np.linalg.norm(th_a - th0)     # same trajectory up to the order of atomic sums
+
+
+def _two_species_equal_shape_problem():
+    """Four 128-atom bcc cells (config 2's recipe) with two species: structures 0, 1 hold 100 + 28 atoms of species 0 / 1, structures
+    2, 3 hold 28 + 100.  The batches [0, 1] and [2, 3] agree in every count the launch shapes depend on (structures, atoms, slices,
+    network tiles) and differ only in where the tiles of species 1 start."""
+    w = wl.make_config(2, n_struct=4, model=wl.ModelSpec(2, 6.0, 4.0, 4, 4, 8, 8, 4, 2, 1, 30))
+    ty = w.structures.type.reshape(4, 128)
+    ty[:2, 100:] = 1
+    ty[2:, 28:] = 1
+    return H.make_problem(w)
+
+
+def test_step_graph_over_equal_shape_batches_of_different_composition():
+    """A captured step graph carries the first network tile of every species by value.  Two mini-batches of the same shape with other
+    atoms per species must not replay each other's graph: the graph path lands on the parameters of the three-call path."""
+    prob = _two_species_equal_shape_problem()
+    lam = (1.0, 1.0, 1.0)
+    A, B = np.array([0, 1], np.int32), np.array([2, 3], np.int32)
+    th = {}
+    for use_graph in (True, False):
+        with H.make_gpu(prob) as nep:
+            th0 = nep.get_params()
+            for ids in (A, A, A, B, B, B, A, B):        # the third step on a batch replays the graph captured at the second
+                nep.set_batch(ids)
+                nep.train_step(*lam, 1e-3, use_graph=use_graph)
+            th[use_graph] = nep.get_params()
+    assert np.linalg.norm(th[True] - th[False]) <= 1e-3 * np.linalg.norm(th[False] - th0)
+
+
+def test_step_graph_after_a_second_neighbour_build():
+    """nep_build_neighbors releases and re-allocates the lists, the pair cache and the slot tables: a step graph captured before it
+    points at freed buffers and has to be captured again (include/nep.h, nep_train_step)."""
+    prob = _prob("tiny_T3_ragged")
+    lam = (1.0, 2.0, 3.0)
+    th = {}
+    for use_graph in (True, False):
+        with H.make_gpu(prob) as nep:
+            th0 = nep.get_params()
+            for _ in range(3):
+                nep.train_step(*lam, 1e-3, use_graph=use_graph)
+            junk = [nep._torch.empty(1 << 20, dtype=nep._torch.uint8, device="cuda") for _ in range(8)]   # noqa: F841  other addresses next time
+            nep.build_neighbors()
+            for _ in range(3):
+                nep.train_step(*lam, 1e-3, use_graph=use_graph)
+            th[use_graph] = nep.get_params()
+    assert np.linalg.norm(th[True] - th[False]) <= 1e-3 * np.linalg.norm(th[False] - th0)
 
 
 def test_empty_batch_and_state_errors():
@@ -253,6 +328,23 @@ def test_compute_scaler_matches_definition(name):
     with H.make_gpu(prob, scaler="compute") as nep:
         s = nep.get_scaler()
     assert np.allclose(s, prob.scaler, rtol=2e-5), np.max(np.abs(s / prob.scaler - 1))
+
+
+def test_compute_scaler_small_descriptors():
+    """Eq. 2 on components that are small but well resolved: with the angular coefficients scaled by 0.05 the 4-/5-body invariants
+    have ranges of 1e-6 ... 2e-8 (below 64 eps_fp32, where an absolute threshold would return 1) and the oracle's 1 / range holds."""
+    prob = _prob("tiny_T3_ragged")
+    th = prob.theta.copy()
+    th[prob.workload.model.block_slices()["cA"]] *= 0.05
+    th = th.astype(np.float32).astype(np.float64)
+    q = O.descriptors(prob.data, th)
+    rng = q.max(axis=0) - q.min(axis=0)
+    assert rng.min() > 1e-8 and np.sum(rng < 64 * 1.2e-7) >= 4
+    with H.make_gpu(prob, labels=False, scaler=None) as nep:
+        nep.set_params(th.astype(np.float32))
+        nep.compute_scaler()
+        s = nep.get_scaler()
+    assert np.allclose(s, O.scaler(q), rtol=1e-4), np.max(np.abs(s / O.scaler(q) - 1))
 
 
 def test_scaler_of_a_perfect_lattice():

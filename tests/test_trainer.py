@@ -92,6 +92,24 @@ def test_rmse_recombines_chunks_with_their_counts():
     assert r["force"] == pytest.approx(np.sqrt(l4[2]), rel=1e-12)
     assert r["virial_per_atom"] == pytest.approx(np.sqrt(l4[3]), rel=1e-12)
     assert min(r.values()) > 0
+    # the counts come from the context: leaving the mask out gives the same report (the labels carry it) ...
+    r2 = T.Trainer(nep, T.TrainConfig()).rmse(chunk=4)
+    assert r2 == r
+    # ... a mask that contradicts the loaded one is refused, and a context without batch_counts() still works from the arguments
+    with pytest.raises(ValueError):
+        T.Trainer(nep, T.TrainConfig()).rmse(st.n_atoms, has_virial=np.ones(6, np.uint8), chunk=4)
+
+    class NoCounts:
+        def __init__(self, inner):
+            self._i = inner
+            self.n_struct = inner.n_struct
+
+        def __getattr__(self, name):
+            if name == "batch_counts":
+                raise AttributeError(name)
+            return getattr(self._i, name)
+    r3 = T.Trainer(NoCounts(nep), T.TrainConfig()).rmse(st.n_atoms, has_virial=hv, chunk=4)
+    assert r3 == r
 
 
 @pytest.mark.gpu
@@ -129,7 +147,7 @@ def test_trajectory_matches_oracle_and_loss_decreases():
         # RMSE report = sqrt of the mean squares of Eqs. 5-7 over the whole set, against the oracle at the trained parameters
         hv = (np.arange(st.n_struct) % 3 != 1).astype(np.uint8)
         nep.set_labels(prob.E, prob.F, prob.W, hv)
-        r = tr2.rmse(st.n_atoms, has_virial=hv, chunk=3)                 # three chunks of unequal size (3, 3, 2)
+        r = tr2.rmse(chunk=3)                 # three chunks of unequal size (3, 3, 2); the mask is the one given to set_labels
         prob.data.set_labels(prob.E, prob.F, prob.W, hv)
         try:
             l4o, _ = O.loss_grad(prob.data, nep.get_params().astype(np.float64), prob.scaler, (1.0, 1.0, 1.0), want_grad=False)
