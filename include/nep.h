@@ -177,6 +177,21 @@ int nep_set_batch(nep_ctx* ctx, int n, const int* struct_ids);
  * Results are kept inside the context for nep_loss_grad. */
 int nep_forward(nep_ctx* ctx, void* E_out, void* F_out, void* W_out, int outputs_on_host);
 
+/* Short-range pair correction ("TorchNEP fully supports the Ziegler-Biersack-Littmark (ZBL) potential [24] as a short-range
+ * correction").  The paper prints neither the screening constants nor the switching radii, so the library stores
+ * none: the term has a fixed form, a screened Coulomb repulsion that is switched off smoothly, and the caller supplies every
+ * number in it (DESIGN reading G29):
+ *     E += sum over undirected pairs {(i,0), (j,n)} with r < r_outer of  phi_ij(r),
+ *     phi_ij(r) = sw(r) (coulomb_k Z_i Z_j / r) sum_{m < n_terms} coef[m] exp(-expo[m] r / a_ij),  a_ij = a_prefac / (Z_i^a_pow + Z_j^a_pow),
+ *     sw(r) = 1 for r <= r_inner, 1/2 (1 + cos(pi (r - r_inner) / (r_outer - r_inner))) up to r_outer, 0 beyond.
+ * Z [n_species] > 0 (host); 0 <= r_inner < r_outer <= rc_R (Angstrom); 1 <= n_terms <= 8, expo >= 0 (host arrays, copied);
+ * a_prefac > 0 (Angstrom); coulomb_k = e^2 / (4 pi eps_0) in eV Angstrom.  From then on nep_forward adds the term to E, F and W
+ * (F = -dE/dr, W = -sum d (x) dE/dd); nep_loss_grad sees the corrected predictions; the term holds no model parameter, so it adds
+ * nothing to the gradient by itself.  Z == NULL or n_terms == 0 switches it off.  Not written to model files.  Invalidates the
+ * step graph and the forward results.  NEP_EINVAL / NEP_ECAPACITY for arguments outside the ranges above. */
+int nep_set_pair_correction(nep_ctx* ctx, const double* Z, double r_inner, double r_outer, int n_terms, const double* coef,
+                            const double* expo, double a_prefac, double a_pow, double coulomb_k);
+
 /* Unscaled descriptors q [N_b][D] (float, host) of the current batch, from the last nep_forward. */
 int nep_get_descriptors(nep_ctx* ctx, float* q);
 

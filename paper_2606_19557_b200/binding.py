@@ -53,6 +53,7 @@ SIGNATURES = {
     "nep_scaler_static": (C.c_int, [_P, C.c_int64, C.c_int, _P, _P]),
     "nep_set_batch": (C.c_int, [_P, C.c_int, _P]),
     "nep_forward": (C.c_int, [_P, _P, _P, _P, C.c_int]),
+    "nep_set_pair_correction": (C.c_int, [_P, _P, C.c_double, C.c_double, C.c_int, _P, _P, C.c_double, C.c_double, C.c_double]),
     "nep_get_descriptors": (C.c_int, [_P, _P]),
     "nep_loss_grad": (C.c_int, [_P, C.c_double, C.c_double, C.c_double, _P]),
     "nep_get_loss": (C.c_int, [_P, _P]),
@@ -404,6 +405,15 @@ class Nep:
         """S1-S5 without synchronising.  E, F, W: optional float32 CUDA tensors receiving the outputs."""
         dp = lambda t: None if t is None else C.c_void_p(t.data_ptr())   # noqa: E731
         self._ck(self._L.nep_forward(self._h, dp(E), dp(F), dp(W), 0))
+
+    def set_pair_correction(self, Z=None, r_inner=0.0, r_outer=0.0, coef=(), expo=(), a_prefac=1.0, a_pow=1.0, coulomb_k=1.0):
+        """nep_set_pair_correction: the short-range pair term of P:105 with the caller's constants; Z=None switches it off."""
+        if Z is None:
+            self._ck(self._L.nep_set_pair_correction(self._h, None, 0.0, 0.0, 0, None, None, 1.0, 1.0, 1.0))
+            return
+        Z = _np(Z, np.float64, (self.get_model()["n_species"],)); coef = _np(coef, np.float64); expo = _np(expo, np.float64, (len(coef),))
+        self._ck(self._L.nep_set_pair_correction(self._h, _ptr(Z), float(r_inner), float(r_outer), len(coef), _ptr(coef), _ptr(expo),
+                                                 float(a_prefac), float(a_pow), float(coulomb_k)))
 
     def get_descriptors(self) -> np.ndarray:
         Sb, Nb = self.batch_shape()

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnep_b200.so")
 SOURCES = ["nep_api.cu", "nep_neighbor.cu", "nep_ang_fwd.cu", "nep_ang_force.cu", "nep_ang_tangent.cu", "nep_ang_adjoint.cu",
-           "nep_radial.cu", "nep_ann.cu", "nep_ann_tc.cu", "nep_misc.cu", "nep_adam.cu", "nep_graph.cu", "nep_static.cu", "nep_peak.cu"]
+           "nep_radial.cu", "nep_ann.cu", "nep_ann_tc.cu", "nep_misc.cu", "nep_adam.cu", "nep_graph.cu", "nep_static.cu", "nep_peak.cu", "nep_pair.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 # the neighbour predicate must be bit-reproducible against the oracle: no FMA contraction in that unit

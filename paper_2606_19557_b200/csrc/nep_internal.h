@@ -101,6 +101,17 @@ struct BatchDev {
     unsigned* counter;   // [64] [0]: block ticket of the loss kernel
 };
 
+// Short-range pair correction (DESIGN G29): phi_ij(r) = sw(r) pref[ti][tj] / r sum_m coef_m exp(-expo_m r ainv[ti][tj]).
+// Every number is the caller's (nep_set_pair_correction); passed to the kernel by value.
+constexpr int MAX_PAIR_TERMS = 8;
+struct PairCorrDev {
+    int n_terms;
+    float r_inner, r_outer, inv_width;       // inv_width = 1 / (r_outer - r_inner)
+    float coef[MAX_PAIR_TERMS], expo[MAX_PAIR_TERMS];
+    float pref[MAX_T * MAX_T];               // k_C Z_i Z_j
+    float ainv[MAX_T * MAX_T];               // (Z_i^p + Z_j^p) / a_prefac
+};
+
 struct Profiler {
     bool on = false;
     bool paused = false;   // events are skipped while paused (the accumulators are kept)
@@ -154,6 +165,7 @@ struct nep_ctx {
 
     int64_t launches = 0;
     nep::Profiler prof;
+    bool pair_on = false; nep::PairCorrDev pair{};   // short-range pair correction added to E, F, W by nep_forward (nep_pair.cu)
 
     // one training step as a CUDA graph (nep_graph.cu); graph_gen is bumped by every call that changes pointers or launch shapes
     cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr; cudaStream_t cap_stream = nullptr;
@@ -192,6 +204,7 @@ int launch_scaler_from_range(nep_ctx* c, const float* d_rng, float* d_s);   //  
 int launch_gather_outputs(nep_ctx* c, float* dE, float* dF, float* dW);  // nep_misc.cu: slice-blocked -> batch order
 int launch_gather_q(nep_ctx* c, float* dq);                    // [N_b][D]
 int launch_build_alist(nep_ctx* c);                            // nep_misc.cu     : type-sorted atom list of the batch
+int launch_pair_correction(nep_ctx* c);                        // nep_pair.cu     : short-range pair term added to E_s, F, W_s (after the force sweeps)
 void graph_drop(nep_ctx* c);                                   // nep_graph.cu    : releases the captured step graph
 int ann_tile_m(const nep_ctx* c);                              // nep_ann.cu      : atoms per network tile for this model
 

@@ -291,7 +291,8 @@ int launch_forward(nep_ctx* c, bool descriptors_only)
     f.back();
     if (!rc) rc = launch_ang_force(c, a);              // S5 angular
     const int rj = f.join();
-    return rc ? rc : rj;
+    if (rc || rj) return rc ? rc : rj;
+    return c->pair_on ? launch_pair_correction(c) : NEP_OK;   // short-range pair term, only when the caller set one
 }
 
 int launch_loss_grad(nep_ctx* c)
