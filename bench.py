@@ -469,14 +469,14 @@ def run_ours(args):
         roof["kernel_sum_over_step"] = (ksum / max(n_prof, 1)) / (total_ms / K)
         roof["duration_source"] = "CUDA events around each kernel in a separate pass of steps (three calls, not the graph); see kernel_sum_over_step"
         roof["traffic"] = None
-        tpath = os.path.join(ROOT, "profiles", "r02_traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
+        tpath = os.path.join(ROOT, "profiles", "r03_traffic.json")   # DRAM bytes per launch from the committed ncu --set full capture
         if os.path.exists(tpath):
             tj = json.load(open(tpath))
             if tj.get("csrc_sha") != rf.csrc_hash():
-                roof["traffic_source"] = "none: the kernel sources changed after the capture in profiles/r02_traffic.json"
+                roof["traffic_source"] = "none: the kernel sources changed after the capture in profiles/r03_traffic.json"
             elif tj.get("workload") == f"config{w.config_id}" and args.n_struct is None and world == 1:
                 roof["traffic"] = tj["bytes_per_launch"].get(top)
-                roof["traffic_source"] = tj.get("source", "profiles/r02_summary.md") + " (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
+                roof["traffic_source"] = tj.get("source", "profiles/r03_summary.md") + " (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
         roof["share_of_step"] = kern[top]["share"]
         roof["avg_ms"] = kern[top]["ms"]
         roof["algorithmic_flops_per_launch"] = mdl["flops"]
